@@ -1,0 +1,185 @@
+/*
+ * mss.h -- C ABI of the B200-native MaxSSmap hot path (arXiv 1403.2136, Turki & Roshan).
+ *
+ * What the library computes (citations are /root/reference/PAPER.md lines; readings in DESIGN.md section 3):
+ *
+ *   mss_genome_load   PAPER.md:55, :69 (sections 2.2.1, 2.2.2): "MaxSSmap divides the genome into fragments of a
+ *                     fixed size given by the user"; "if the genome is not a multiple of the fragment length we pad
+ *                     the last fragment with N's"; the genome is transferred "just once".
+ *   mss_map_reads     PAPER.md:41, :57 (sections 2.1.1, 2.2.1): for every read, the maximum scoring subsequence of
+ *                     the per-base match/mismatch scores of the read laid gap-free at every window start of every
+ *                     fragment ("sliding window", reading into neighbouring fragments to map across junctions);
+ *                     "it outputs the fragment number with the highest and second highest score".
+ *   mss_nw_align      PAPER.md:59, :91: "we align the read sequence with Needleman-Wunsch to the genome region from
+ *                     the first part", match 5, mismatch -4, gap -26.
+ *   mss_mapq_filter   PAPER.md:57, :63: mapped iff second/best < 0.9; MAPQ = -100 log2(second/best).
+ *
+ * Conventions
+ *   - Every pointer named d_* is DEVICE memory owned by the caller; h_* is HOST memory owned by the caller.
+ *     The library allocates no device memory: scratch comes from the caller through the *_workspace_bytes queries.
+ *     mss_genome_load allocates one small host struct (the handle), released by mss_genome_free; the packed genome
+ *     and the genome workspace must outlive the handle.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls enqueue work on it and
+ *     return; outputs are valid once the caller has synchronised the stream.  The *_host entry points are the
+ *     exception: they copy host buffers in, run, copy results out and synchronise before returning.
+ *   - Return value: 0 (MSS_OK) or a negative mss_status.  No exception or abort crosses this boundary and there is
+ *     no CPU fallback: without a CUDA device every compute call returns MSS_ERR_CUDA.
+ *
+ * Packed sequence format (genome and reads)
+ *   base codes A=0 C=1 G=2 T=3 (complement = code XOR 3); base i sits in bits [2*(i%16), 2*(i%16)+2) of uint32 word
+ *   i/16.  N mask: bit (i%32) of uint32 word i/32, 1 = N; the 2-bit code under an N is ignored.  A NULL mask means
+ *   "no N".  Genome arrays hold ceil(n_bases/16) and ceil(n_bases/32) words.  Reads are rows of
+ *   `read_stride_words` words (>= ceil(max_len/16)); their mask rows have ceil(read_stride_words/2) words; bits
+ *   beyond len[r] are ignored.
+ */
+#ifndef MSS_H
+#define MSS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mss_genome mss_genome_t;                          /* opaque handle */
+
+typedef struct { int32_t match, mismatch, gap; } mss_scoring_t;  /* paper defaults 5, -4, -26;
+                                                                    N against anything (N included) = mismatch */
+
+typedef struct { int32_t frag, diag, score, strand; } mss_hit_t; /* frag: fragment index, -1 = no such fragment;
+                                                                    diag: window start inside the fragment, [0, F);
+                                                                    strand: 0 forward, 1 reverse-complemented read */
+typedef struct { mss_hit_t best, second; } mss_top2_t;           /* 32 bytes per read */
+
+enum { MSS_FWD = 1, MSS_REV = 2, MSS_BOTH = 3 };                 /* `strands` argument */
+enum { MSS_OVERLAP_PAPER = -1 };                                 /* look-ahead = read length - 1, per read */
+
+typedef enum {
+    MSS_OK = 0,
+    MSS_ERR_ARG = -1,        /* NULL pointer, n_bases <= 0, frag_len <= 0, overlap < -1, n_reads < 0, stride too small,
+                                strands not in {1,2,3}, pad < 0, cigar_stride < 1 */
+    MSS_ERR_RANGE = -2,      /* match <= 0, mismatch >= 0, gap >= 0, max_len*match > 32767, mismatch < -32768,
+                                frag_len > 2^24, number of fragments > 2^31-1, max_len > MSS_MAX_READ_LEN */
+    MSS_ERR_WORKSPACE = -3,  /* workspace_bytes smaller than the matching *_workspace_bytes query */
+    MSS_ERR_CUDA = -4        /* no device, launch failure, or any CUDA runtime error (see mss_last_cuda_error) */
+} mss_status;
+
+#define MSS_MAX_READ_LEN 6553   /* floor(32767 / 5): packed 16-bit score lanes stay exact; checked against match */
+
+/* ---- genome -------------------------------------------------------------------------------------------------- */
+
+/* Bytes of device scratch mss_genome_load needs for a genome of n_bases (0 on bad arguments). */
+size_t mss_genome_workspace_bytes(int64_t n_bases, int32_t frag_len, int32_t overlap);
+
+/*
+ * Derive the scan layout from the caller's packed genome.
+ *   d_packed, d_nmask  packed genome and N mask (d_nmask may be NULL), n_bases bases.
+ *   frag_len F >= 1    fragment f owns window starts [f*F, f*F+F); nfrag = ceil(n_bases/F); positions >= n_bases
+ *                      behave as N.
+ *   overlap V          bases past the fragment end a window may read: MSS_OVERLAP_PAPER (-1) = read length - 1
+ *                      (the read is always "fully mapped"), V >= 0 = min(V, read length - 1).
+ *   d_workspace        >= mss_genome_workspace_bytes(...) bytes, 16-byte aligned; owned by the caller, must outlive
+ *                      the handle.
+ * On success *out receives the handle.
+ */
+int mss_genome_load(const uint32_t *d_packed, const uint32_t *d_nmask, int64_t n_bases,
+                    int32_t frag_len, int32_t overlap, void *d_workspace, size_t workspace_bytes,
+                    void *stream, mss_genome_t **out);
+int mss_genome_free(mss_genome_t *g);
+int32_t mss_genome_num_fragments(const mss_genome_t *g);
+int64_t mss_genome_num_bases(const mss_genome_t *g);
+
+/* ---- first phase: MaxSS scan + top-2 -------------------------------------------------------------------------- */
+
+size_t mss_map_workspace_bytes(const mss_genome_t *g, int32_t n_reads, int32_t max_len, int32_t strands);
+
+/*
+ * For every read r in [0, n_reads): score(f, strand, d) = max(0, best gap-free run) computed as
+ *     H = 0; for i in [0, len[r]): stop if f*F+d+i >= f*F+F+Veff; H = max(0, H + s(read[i], genome[f*F+d+i])); best = max(best, H)
+ * for every fragment f, enabled strand and window start d in [0,F); each fragment is represented by
+ * its maximum (ties: forward strand first, then lowest d); d_out[r] = the two best *distinct* fragments (ties:
+ * lowest fragment index; a fragment scoring 0 is still a fragment; with one fragment second.frag = -1).
+ *   d_reads / d_reads_nmask / read_stride_words / d_lens: packed reads as described above, 1 <= len[r] <= max_len.
+ *   max_len            upper bound of d_lens[] known to the host (sizes shared memory and the score-range check).
+ *   sc                 match > 0 > mismatch; sc.gap is ignored here.
+ *   strands            MSS_FWD, MSS_REV (reverse-complemented read against the forward genome) or MSS_BOTH.
+ * Reads whose length lies outside [1, max_len] get best.frag = second.frag = -1.
+ */
+int mss_map_reads(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
+                  int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
+                  mss_scoring_t sc, int32_t strands, void *d_workspace, size_t workspace_bytes,
+                  void *stream, mss_top2_t *d_out);
+
+/* ---- second phase: Needleman-Wunsch of each read against its best region --------------------------------------- */
+
+size_t mss_nw_workspace_bytes(const mss_genome_t *g, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t pad);
+
+/*
+ * Fitting alignment (all of the read, any substring of the window; linear gap) of read r, reverse-complemented if
+ * d_hits[r].best.strand = 1, against genome[ws, we): ws = max(0, f*F - pad), we = min(n_bases, f*F + F + Veff + pad),
+ * f = d_hits[r].best.frag ("the region of the genome starting from the identified fragment and
+ * spanning fragments to the right").  D[0][j] = 0, D[i][0] = i*gap,
+ * D[i][j] = max(D[i-1][j-1] + s, D[i-1][j] + gap, D[i][j-1] + gap); score = max_j D[len][j], smallest such j;
+ * traceback prefers diagonal (M, op 0), then up (I, op 1), then left (D, op 2).
+ *   d_score[r], d_ref_pos[r] (0-based forward-genome position of the first window base used; ws + end column if
+ *   none), d_cigar[r*cigar_stride ...] = BAM-style (len << 4 | op) in read order, d_n_cigar[r] = number of ops
+ *   (ops beyond cigar_stride are counted but not written).  Reads with best.frag < 0: score 0, pos -1, 0 ops.
+ */
+int mss_nw_align(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
+                 int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
+                 const mss_top2_t *d_hits, mss_scoring_t sc, int32_t pad,
+                 void *d_workspace, size_t workspace_bytes, void *stream,
+                 int32_t *d_score, int64_t *d_ref_pos, uint32_t *d_cigar, int32_t cigar_stride, int32_t *d_n_cigar);
+
+/* ---- repeat filter and mapping quality ------------------------------------------------ */
+
+/*
+ * d_mapped[r] = 1 iff best.frag >= 0, best.score > 0 and MAPQ > mapq_threshold, where the ratio p = second/best
+ * (second.frag < 0 or second.score = 0 -> p = 0, MAPQ = +inf reported as 3.4e38) and MAPQ = -100 log2 p (float32).
+ * The paper's default threshold is -100 log2 0.9 = 15.2; the integer form 10*second < 9*best decides at exactly 15.2
+ * (pass mapq_threshold < 0 to use that exact integer rule).  d_mapq may be NULL.
+ */
+int mss_mapq_filter(const mss_top2_t *d_hits, int32_t n_reads, float mapq_threshold,
+                    void *stream, uint8_t *d_mapped, float *d_mapq);
+
+/* ---- end-to-end convenience with HOST buffers (used for the e2e timing of bench.py) ---------------------------- */
+
+/*
+ * Same as mss_map_reads, but reads, lengths and output are HOST pointers: copies them to the device workspace,
+ * scans, copies the n_reads records back and synchronises.  d_workspace must hold
+ * mss_map_host_workspace_bytes(...) bytes.
+ */
+size_t mss_map_host_workspace_bytes(const mss_genome_t *g, int32_t n_reads, int32_t max_len, int32_t read_stride_words,
+                                    int32_t strands);
+int mss_map_reads_host(const mss_genome_t *g, const uint32_t *h_reads, const uint32_t *h_reads_nmask,
+                       int32_t read_stride_words, const int32_t *h_lens, int32_t n_reads, int32_t max_len,
+                       mss_scoring_t sc, int32_t strands, void *d_workspace, size_t workspace_bytes,
+                       void *stream, mss_top2_t *h_out);
+
+/* ---- diagnostics ------------------------------------------------------------------------------------------------ */
+
+const char *mss_strerror(int status);
+int mss_last_cuda_error(void);                 /* cudaError_t of the last MSS_ERR_CUDA on this thread, 0 if none */
+int mss_version(void);                         /* 100*major + minor */
+
+/*
+ * Tuning / introspection (does not change results): select the scan kernel variant (0 = automatic) and report the
+ * launch geometry of the last mss_map_reads call on this thread.  Used by bench.py and the parity tests to cover
+ * every variant.
+ */
+int mss_set_scan_variant(int variant);
+typedef struct { int32_t variant, grid, block, smem_bytes, reads_per_block, tile_diagonals, launches; } mss_launch_info_t;
+int mss_get_last_launch(mss_launch_info_t *out);
+
+/*
+ * Live measurement of the integer/DPX issue peak the scan's roofline is quoted against: runs `iters` dependent
+ * rounds of 8 independent VIADDMNMX.S16x2.RELU / VIMNMX3.S16x2 chains (2:1 mix, the scan's own DPX mix) per thread
+ * on every SM and returns thread-instructions per second in *h_instr_per_s and the elapsed ms in *h_ms.
+ */
+int mss_probe_dpx_peak(int32_t iters, void *stream, double *h_instr_per_s, float *h_ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MSS_H */

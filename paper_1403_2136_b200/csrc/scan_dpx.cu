@@ -1,0 +1,296 @@
+// a1-a6: the MaxSS scan as genome-tile x read-batch blocks with packed 16-bit DPX lanes.
+//
+// What a block does (one work unit = a group of reads x a range of fragments):
+//   once:      a1 read prep -- for every query (read, strand) a row-offset table roff[i] = base(i)*ROWW + i
+//   per tile:  a2 stage the tile: D = 2*K*T window starts [g0, g0+D) of one fragment plus the m-1 look-ahead are
+//              turned into 5 "score planes" in shared memory: plane[c][x] = the s16x2 pair
+//              ( s(c, G[g0+x]) , s(c, G[g0+x+D/2]) ), c in {A,C,G,T,N}; N / beyond-the-window positions score mismatch
+//              (PAPER.md:69 padding; readings 5, 6)
+//   per query: a3 Kadane -- thread t owns K lane pairs = window starts {kT+t, kT+t+D/2}; step i is
+//                  H_k = max(H_k + plane[read[i]][kT+t+i], 0)       one LDS.32 + one VIADDMNMX.S16x2.RELU per 2 cells
+//                  B_k = max(B_k, H_k(i), H_k(i+1))                  one VIMNMX3.S16x2 per 4 cells
+//              ("maximum scoring subsequence"; the paper's look-ahead of 16 windows, becomes
+//              2K windows per thread held in registers)
+//              a4 fragment max: warp REDUX max + lowest window start, one slot per (query, warp)
+//   per tile:  fold the per-warp slots into the read's running fragment candidate (score desc, strand asc, diag asc);
+//              at the last tile of a fragment push it into the read's top-2 (a5, strictly greater, fragments ascending)
+//   at end:    a6 emit the read's top-2 (or the unit's partial top-2, merged by top2_merge_kernel)
+#include "mss_common.cuh"
+
+namespace {
+
+struct DpxUnitGeom {
+    int32_t n_groups, n_splits, frags_per_split, reads_per_group;
+};
+
+template <int K, int T>
+struct Cfg {
+    static constexpr int HALF = K * T;
+    static constexpr int D = 2 * K * T;
+    static constexpr int NW = T / 32;
+};
+
+constexpr int NQ_MAX = 32;          // queries (read x strand) per block
+
+__device__ __forceinline__ uint32_t pack2(int32_t lo, int32_t hi)
+{
+    return ((uint32_t)lo & 0xFFFFu) | ((uint32_t)hi << 16);
+}
+
+template <int K, int T>
+__global__ void __launch_bounds__(T)
+scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2_t* __restrict__ out_partial)
+{
+    using C = Cfg<K, T>;
+    extern __shared__ __align__(16) uint32_t smem[];
+    uint32_t* planes = smem;                                   // 5 * ROWW
+    uint32_t* roff = planes + 5 * ROWW;                        // NQ_MAX * MP
+    uint32_t* wres = roff + NQ_MAX * MP;                       // NQ_MAX * NW
+    int32_t* qlen = (int32_t*)(wres + NQ_MAX * C::NW);         // NQ_MAX
+    unsigned long long* cur = (unsigned long long*)(qlen + NQ_MAX);   // NQ_MAX (per read; 8-byte aligned by layout)
+    mss_hit_t* tbest = (mss_hit_t*)(cur + NQ_MAX);             // NQ_MAX
+    mss_hit_t* tsecond = tbest + NQ_MAX;                       // NQ_MAX
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int32_t group = blockIdx.x % ug.n_groups, split = blockIdx.x / ug.n_groups;
+    const int32_t ns = (p.strands == 3) ? 2 : 1;
+    const int32_t r0 = group * ug.reads_per_group;
+    const int32_t nr = min(ug.reads_per_group, p.n_reads - r0);
+    const int32_t nq = nr * ns;
+    const int32_t f_begin = split * ug.frags_per_split;
+    const int32_t f_end = min(p.n_frag, f_begin + ug.frags_per_split);
+
+    // ---- a1: read prep ------------------------------------------------------------------------------------------
+    for (int32_t q = warp; q < nq; q += C::NW) {
+        int32_t r = r0 + q / ns;
+        int32_t strand = (ns == 2) ? (q & 1) : (p.strands == 2 ? 1 : 0);
+        int32_t m = p.lens[r];
+        bool ok = (m >= 1 && m <= p.max_len);
+        const uint32_t* rw = p.reads + (int64_t)r * p.stride_words;
+        const uint32_t* rn = p.reads_nmask ? p.reads_nmask + (int64_t)r * ((p.stride_words + 1) / 2) : nullptr;
+        for (int32_t i = lane; i < MP; i += 32) {
+            uint32_t b = (ok && i < m) ? read_base(rw, rn, m, i, strand) : 4u;
+            roff[q * MP + i] = (b * (uint32_t)ROWW + (uint32_t)i) * 4u;      // byte offset into the planes
+        }
+        if (lane == 0) qlen[q] = ok ? m : 0;
+    }
+    if (tid < NQ_MAX) {
+        cur[tid] = 0ull;
+        mss_hit_t none = { -1, 0, 0, 0 };
+        tbest[tid] = none;
+        tsecond[tid] = none;
+    }
+
+    const char* my = reinterpret_cast<const char*>(planes + tid);
+    const uint32_t zero = (uint32_t)p.zero;                     // opaque 0: keeps ptxas from re-materialising it per use
+    const int32_t tiles_per_frag = (p.F + C::D - 1) / C::D;
+
+    for (int32_t f = f_begin; f < f_end; f++) {
+        const int64_t fstart = (int64_t)f * p.F;
+        const int64_t trunc = (p.V < 0) ? (int64_t)0x7FFFFFFFFFFFFFFFll : fstart + p.F + p.V;   // positions >= trunc are not readable
+        for (int32_t tile = 0; tile < tiles_per_frag; tile++) {
+            const int32_t toff = tile * C::D;
+            const int64_t g0 = fstart + toff;
+            const int32_t nvalid = min(C::D, p.F - toff);
+            __syncthreads();                                    // previous tile fully scanned and folded
+            // ---- a2: stage the tile as score planes ------------------------------------------------------------
+            for (int32_t x = tid; x < ROWW; x += T) {
+                int64_t plo = g0 + x, phi = plo + C::HALF;
+                uint32_t lo = plo < trunc ? base_at(p.gpacked, p.gnmask, plo) : 4u;
+                uint32_t hi = phi < trunc ? base_at(p.gpacked, p.gnmask, phi) : 4u;
+#pragma unroll
+                for (uint32_t c = 0; c < 4; c++)
+                    planes[c * ROWW + x] = pack2(lo == c ? p.match : p.mismatch, hi == c ? p.match : p.mismatch);
+                planes[4 * ROWW + x] = pack2(p.mismatch, p.mismatch);
+            }
+            __syncthreads();
+
+            // ---- a3/a4: every query against the tile -----------------------------------------------------------
+            for (int32_t q = 0; q < nq; q++) {
+                const int32_t m = qlen[q];
+                if (m == 0) { if (lane == 0) wres[q * C::NW + warp] = 0u; continue; }
+                const uint32_t* ro = roff + q * MP;
+                uint32_t H[K], B[K];
+#pragma unroll
+                for (int k = 0; k < K; k++) { H[k] = 0u; B[k] = 0u; }
+                for (int32_t i0 = 0; i0 < m; i0 += 4) {
+                    const uint4 o = *reinterpret_cast<const uint4*>(ro + i0);
+                    uint32_t Ha[K];
+#pragma unroll
+                    for (int k = 0; k < K; k++) Ha[k] = __viaddmax_s16x2(H[k], *reinterpret_cast<const uint32_t*>(my + o.x + k * T * 4), zero);
+#pragma unroll
+                    for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.y + k * T * 4), zero);
+#pragma unroll
+                    for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+#pragma unroll
+                    for (int k = 0; k < K; k++) Ha[k] = __viaddmax_s16x2(H[k], *reinterpret_cast<const uint32_t*>(my + o.z + k * T * 4), zero);
+#pragma unroll
+                    for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.w + k * T * 4), zero);
+#pragma unroll
+                    for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                }
+                // a4: warp max and its lowest window start
+                if (nvalid < C::D) {                            // ragged last tile of a fragment: drop foreign window starts
+#pragma unroll
+                    for (int k = 0; k < K; k++) {
+                        int dlo = k * T + tid;
+                        if (dlo >= nvalid) B[k] &= 0xFFFF0000u;
+                        if (dlo + C::HALF >= nvalid) B[k] &= 0x0000FFFFu;
+                    }
+                }
+                uint32_t mx = B[0];
+#pragma unroll
+                for (int k = 1; k < K; k++) mx = __vmaxs2(mx, B[k]);
+                uint32_t M = max(mx & 0xFFFFu, mx >> 16);
+                uint32_t W = __reduce_max_sync(0xffffffffu, M);
+                uint32_t d = 0xFFFFu;
+                if (M == W) {
+#pragma unroll
+                    for (int k = K - 1; k >= 0; k--) if ((B[k] >> 16) == W) d = (uint32_t)(k * T + tid + C::HALF);
+#pragma unroll
+                    for (int k = K - 1; k >= 0; k--) if ((B[k] & 0xFFFFu) == W) d = (uint32_t)(k * T + tid);
+                }
+                d = __reduce_min_sync(0xffffffffu, d);
+                if (lane == 0) wres[q * C::NW + warp] = (W << 16) | (0xFFFFu - d);
+            }
+            __syncthreads();
+            // ---- fold into the running fragment candidate; a5 top-2 at the fragment's last tile ------------------
+            if (tid < nr) {
+                unsigned long long c = cur[tid];
+                for (int32_t s = 0; s < ns; s++) {
+                    int32_t q = tid * ns + s;
+                    if (qlen[q] == 0) continue;
+                    uint32_t best = 0u;
+                    for (int w = 0; w < C::NW; w++) best = max(best, wres[q * C::NW + w]);
+                    int32_t strand = (ns == 2) ? s : (p.strands == 2 ? 1 : 0);
+                    unsigned long long k64 = frag_key((int32_t)(best >> 16), strand, toff + (int32_t)(0xFFFFu - (best & 0xFFFFu)));
+                    c = k64 > c ? k64 : c;
+                }
+                if (tile == tiles_per_frag - 1) {
+                    if (c != 0ull) {
+                        mss_hit_t h; h.frag = f;
+                        frag_key_unpack(c, h.score, h.strand, h.diag);
+                        mss_hit_t b = tbest[tid], s2 = tsecond[tid];
+                        top2_push(b, s2, h);
+                        tbest[tid] = b; tsecond[tid] = s2;
+                    }
+                    c = 0ull;
+                }
+                cur[tid] = c;
+            }
+        }
+    }
+    __syncthreads();
+    if (tid < nr) {
+        mss_top2_t o; o.best = tbest[tid]; o.second = tsecond[tid];
+        out_partial[(int64_t)split * p.n_reads + r0 + tid] = o;
+    }
+}
+
+__global__ void top2_merge_kernel(const mss_top2_t* __restrict__ partial, int32_t n_splits, int32_t n_reads,
+                                  mss_top2_t* __restrict__ out)
+{
+    int32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_reads) return;
+    mss_hit_t none = { -1, 0, 0, 0 };
+    mss_hit_t best = none, second = none;
+    for (int32_t s = 0; s < n_splits; s++) {
+        mss_top2_t t = partial[(int64_t)s * n_reads + r];
+        top2_merge(best, second, t.best);
+        top2_merge(best, second, t.second);
+    }
+    out[r].best = best;
+    out[r].second = second;
+}
+
+DpxUnitGeom unit_geom(const mss_genome* g, int32_t n_reads, int32_t strands)
+{
+    DpxUnitGeom ug;
+    int32_t ns = strands == 3 ? 2 : 1;
+    ug.reads_per_group = NQ_MAX / ns;
+    ug.n_groups = (n_reads + ug.reads_per_group - 1) / ug.reads_per_group;
+    if (ug.n_groups < 1) ug.n_groups = 1;
+    int64_t target = (int64_t)g->sm_count * 32;
+    int64_t want = (target + ug.n_groups - 1) / ug.n_groups;
+    if (want < 1) want = 1;
+    if (want > g->n_frag) want = g->n_frag;
+    if (want > 4096) want = 4096;
+    ug.frags_per_split = (int32_t)((g->n_frag + want - 1) / want);
+    ug.n_splits = (g->n_frag + ug.frags_per_split - 1) / ug.frags_per_split;
+    return ug;
+}
+
+struct Variant { int id, K, T; };
+const Variant kVariants[] = { {2, 8, 256}, {3, 8, 128}, {4, 8, 64}, {5, 4, 256}, {6, 16, 128} };
+
+template <int K, int T>
+cudaError_t launch_variant(const mss_genome* g, const ScanParams& p, const DpxUnitGeom& ug, mss_top2_t* partial,
+                           cudaStream_t st, mss_launch_info_t* info, int id)
+{
+    using C = Cfg<K, T>;
+    int32_t MP = (p.max_len + 3) & ~3;
+    int32_t ROWW = (C::HALF + MP + 3) & ~3;
+    size_t smem = (size_t)(5 * ROWW + NQ_MAX * MP + NQ_MAX * C::NW) * 4 + NQ_MAX * 4 + NQ_MAX * 8 + 2 * NQ_MAX * sizeof(mss_hit_t);
+    if (smem > (size_t)g->max_smem_optin) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute(scan_dpx_kernel<K, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int64_t blocks = (int64_t)ug.n_groups * ug.n_splits;
+    scan_dpx_kernel<K, T><<<(unsigned)blocks, T, smem, st>>>(p, ug, MP, ROWW, partial);
+    if (info) {
+        info->variant = id; info->grid = (int32_t)blocks; info->block = T; info->smem_bytes = (int32_t)smem;
+        info->reads_per_block = ug.reads_per_group; info->tile_diagonals = C::D; info->launches = 2;
+    }
+    return cudaGetLastError();
+}
+
+int pick_variant(const mss_genome* g, int requested)
+{
+    for (const Variant& v : kVariants) if (v.id == requested) return requested;
+    // automatic: the tile size with the least padding waste, larger tiles preferred on ties
+    int best = 2; double best_waste = 1e30;
+    for (const Variant& v : kVariants) {
+        if (v.id > 4) continue;                                  // 5, 6 are tuning variants, never automatic
+        int D = 2 * v.K * v.T;
+        double waste = (double)((g->frag_len + D - 1) / D) * D / g->frag_len;
+        if (waste < best_waste - 1e-9) { best_waste = waste; best = v.id; }
+    }
+    return best;
+}
+
+}  // namespace
+
+bool scan_dpx_supported(const mss_genome* g, const ScanParams& p)
+{
+    if (g->frag_len < 256) return false;                        // tiles would be mostly padding: generic kernel
+    if ((int64_t)p.max_len * p.match > 32767 || p.mismatch < -32768) return false;
+    int32_t MP = (p.max_len + 3) & ~3;
+    size_t smem_min = (size_t)(5 * (512 + MP + 4) + NQ_MAX * MP + NQ_MAX * 8) * 4 + 4096;
+    return smem_min <= (size_t)g->max_smem_optin;
+}
+
+size_t scan_dpx_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, int32_t strands)
+{
+    (void)max_len;
+    DpxUnitGeom ug = unit_geom(g, n_reads > 0 ? n_reads : 1, strands);
+    return (size_t)ug.n_splits * (size_t)(n_reads > 0 ? n_reads : 1) * sizeof(mss_top2_t) + 256;
+}
+
+cudaError_t launch_scan_dpx(const mss_genome* g, const ScanParams& p, void* ws, size_t ws_bytes,
+                            mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info, int variant)
+{
+    (void)ws_bytes;
+    DpxUnitGeom ug = unit_geom(g, p.n_reads, p.strands);
+    mss_top2_t* partial = (mss_top2_t*)ws;
+    int id = pick_variant(g, variant);
+    cudaError_t e;
+    switch (id) {
+        case 3: e = launch_variant<8, 128>(g, p, ug, partial, st, info, id); break;
+        case 4: e = launch_variant<8, 64>(g, p, ug, partial, st, info, id); break;
+        case 5: e = launch_variant<4, 256>(g, p, ug, partial, st, info, id); break;
+        case 6: e = launch_variant<16, 128>(g, p, ug, partial, st, info, id); break;
+        default: e = launch_variant<8, 256>(g, p, ug, partial, st, info, 2); break;
+    }
+    if (e != cudaSuccess) return e;
+    top2_merge_kernel<<<(p.n_reads + 255) / 256, 256, 0, st>>>(partial, ug.n_splits, p.n_reads, d_out);
+    return cudaGetLastError();
+}

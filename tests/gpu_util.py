@@ -1,0 +1,32 @@
+"""Helpers for the -m gpu parity tests: marshal gen/ inputs to the device and call the C ABI through the binding."""
+import numpy as np
+
+import gen
+
+
+def to_dev(a, dtype=None):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(a).view(np.int32) if a.dtype == np.uint32 else np.ascontiguousarray(a))
+    return t.cuda()
+
+
+def load_genome(codes, frag_len, overlap):
+    import paper_1403_2136_b200 as mss
+    packed, nmask = gen.pack_2bit(codes)
+    return mss.mss_genome_load(to_dev(packed), to_dev(nmask), int(codes.size), frag_len, overlap)
+
+
+def map_reads(g, reads, lens, strands=3, match=5, mismatch=-4, variant=0, with_mask=True, stride_words=None):
+    import torch
+    import paper_1403_2136_b200 as mss
+    reads = np.asarray(reads, dtype=np.uint8)
+    lens = np.asarray(lens, dtype=np.int32)
+    rp, rn = gen.pack_reads(reads, lens, stride_words)
+    mss.mss_set_scan_variant(variant)
+    try:
+        out = mss.mss_map_reads(g, to_dev(rp), to_dev(rn) if with_mask else None, to_dev(lens), int(reads.shape[1]),
+                                mss.Scoring(match, mismatch, -26), strands)
+        torch.cuda.synchronize()
+    finally:
+        mss.mss_set_scan_variant(0)
+    return out.cpu().numpy()
