@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py -- MaxSS GCUPS of the whole hot path (scan + top-2 + NW) on synthetic config-2 input.
+
+    python bench.py --gpus N --steps K --warmup W            # our CUDA path (C ABI -> libmss.so)
+    python bench.py --impl reference ...                     # the CPU oracle as it stands, on the host cores
+
+A step = one pass of every hot-path stage (read prep, tile staging, Kadane scan, fragment max,
+top-2, emit, NW) over one batch of reads of BASELINE.json's E. coli-sized config (configs[1]); the genome load (a0,
+"once") is timed separately.  One JSON line on stdout (rank 0).  DESIGN.md section 7 explains every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import gen  # noqa: E402
+
+ALGO_INSTR_PER_CELL = 0.75          # 1 VIADDMNMX.S16x2 per 2 cells + 1 VIMNMX3.S16x2 per 4 cells
+ALU_LANES_PER_CLK_SM = 64           # integer/DPX pipe: 16 lanes/clk per SM sub-partition x 4 (guide + measured)
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.proc = index, [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self) -> dict:
+        if self.proc:
+            self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p))
+    return {}
+
+
+def cpu_baseline(cfg, genome, reads, lens, target_s: float = 15.0) -> dict:
+    """The oracle as it stands, on the host cores, on a bounded seeded sample of the same reads."""
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    per_read_cells = cfg.cells() / cfg.n_reads
+    guess = 0.55e9                                   # cells/s/core of the plain -O3 build (measured in DESIGN.md)
+    per_core = max(1, int(target_s * guess / per_read_cells))
+    n = min(reads.shape[0], cores * per_core)
+    t0 = time.perf_counter()
+    oracle.map_reads_parallel(genome, cfg.frag_len, cfg.overlap, reads[:n], lens[:n], strands=cfg.strands, workers=cores)
+    dt = time.perf_counter() - t0
+    cells = per_read_cells * n
+    return {"value": cells / dt / 1e9, "unit": "GCUPS", "cores": min(cores, n), "kind": "oracle",
+            "sample": f"first {n} reads of the step's batch, all {-(-cfg.genome_len // cfg.frag_len)} fragments, both strands, "
+                      f"oracle/maxss_oracle.c -O3 single-threaded per process, {dt:.1f} s wall",
+            "reads_per_s": n / dt}
+
+
+def run_reference(args, cfg):
+    """--impl reference: the CPU oracle timed on this arm's config/metric (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    oracle.build()
+    genome, _ = cfg.genome()
+    cores = os.cpu_count() or 1
+    n = cores * args.ref_reads_per_core
+    r = gen.make_reads(genome, n, cfg.groups[0][1], cfg.reads_seed, sub_rate=cfg.groups[0][2])
+    per_read_cells = cfg.cells() / cfg.n_reads
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        top2 = oracle.map_reads_parallel(genome, cfg.frag_len, cfg.overlap, r["reads"], r["lens"], strands=cfg.strands,
+                                         workers=cores)
+        oracle.nw_align(genome, cfg.frag_len, cfg.overlap, r["reads"][:cores], r["lens"][:cores], top2[:cores])
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * sum(times) / len(times)
+    val = per_read_cells * n / (ms * 1e-3) / 1e9
+    sample = (f"each step: {n} seeded reads of the config ({args.ref_reads_per_core} per core) through the oracle's MaxSS "
+              f"stage on all fragments and both strands, plus its NW on {cores} of them")
+    line = {"impl": "reference", "metric": "MaxSS GCUPS (scan+top-2+NW step)", "value": val, "unit": "GCUPS", "n_gpus": 0,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": f"config {cfg.c} ({cfg.name}) bounded sample", "reads_per_step": n, "read_len": cfg.groups[0][1],
+                       "genome_bp": cfg.genome_len, "frag_len": cfg.frag_len, "overlap": cfg.overlap, "strands": "both"},
+            "cpu_baseline": {"value": val, "unit": "GCUPS", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "GCUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "reads_per_s": n / (ms * 1e-3)}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); the metric is quoted on 2")
+    ap.add_argument("--reads", type=int, default=None, help="reads per step per GPU (default: the config's own count)")
+    ap.add_argument("--variant", type=int, default=0, help="scan kernel variant (0 = automatic)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-nw", action="store_true", help="time the MaxSS stage only (diagnostic; not a bench value)")
+    ap.add_argument("--ref-reads-per-core", type=int, default=2)
+    ap.add_argument("--cigar-stride", type=int, default=16)
+    args = ap.parse_args()
+    cfg = gen.config(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    import paper_1403_2136_b200 as mss
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    # ---- inputs: genome replicated, reads sharded by rank (independent units, no data-path collective) ------------
+    genome, _ = cfg.genome()
+    m = cfg.max_len
+    n_reads = args.reads or cfg.n_reads
+    if args.reads is None:
+        r = cfg.reads(genome) if world == 1 else None
+    else:
+        r = None
+    if r is None:   # ranks draw their own batch (weak scaling): same recipe, seed offset by rank
+        outs = []
+        per = max(1, n_reads // len(cfg.groups))
+        for gi, (_, mm, rate) in enumerate(cfg.groups):
+            o = gen.make_reads(genome, per, mm, cfg.reads_seed + 100 * gi + 7919 * rank, sub_rate=rate,
+                               indel_prob=cfg.indel_prob, both_strands=cfg.both_strands, avoid_n=cfg.avoid_n)
+            if mm < m:
+                pad = np.full((per, m), gen.N, dtype=np.uint8); pad[:, :mm] = o["reads"]; o["reads"] = pad
+            outs.append(o)
+        r = {k: np.concatenate([o[k] for o in outs]) for k in outs[0]}
+    reads, lens = r["reads"], r["lens"]
+    n_reads = reads.shape[0]
+    packed, nmask = gen.pack_2bit(genome)
+    rp, rn = gen.pack_reads(reads, lens)
+    h_reads = torch.from_numpy(rp.view(np.int32)).pin_memory()
+    h_mask = torch.from_numpy(rn.view(np.int32)).pin_memory()
+    h_lens = torch.from_numpy(lens).pin_memory()
+
+    t0 = time.perf_counter()
+    d_packed = torch.from_numpy(packed.view(np.int32)).to(dev)
+    d_nmask = torch.from_numpy(nmask.view(np.int32)).to(dev)
+    G = mss.mss_genome_load(d_packed, d_nmask, int(genome.size), cfg.frag_len, cfg.overlap)
+    torch.cuda.synchronize()
+    genome_load_ms = 1e3 * (time.perf_counter() - t0)
+
+    d_reads, d_mask, d_lens = h_reads.to(dev), h_mask.to(dev), h_lens.to(dev)
+    sc = mss.Scoring()
+    mss.mss_set_scan_variant(args.variant)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)          # > 126 MB L2
+    stream = torch.cuda.current_stream()
+    cells_step = float(np.sum(lens.astype(np.float64))) * G.n_frag * cfg.frag_len * (2 if cfg.strands == 3 else 1)
+
+    def step():
+        """resident inputs -> top-2 records -> NW score/pos/CIGAR, all on the device; returns (scan_ms event pair)."""
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record(stream)
+        top2 = mss.mss_map_reads(G, d_reads, d_mask, d_lens, m, sc, cfg.strands)
+        e1.record(stream)
+        if not args.no_nw:
+            mss.mss_nw_align(G, d_reads, d_mask, d_lens, m, top2, sc, 30, args.cigar_stride)
+        e2.record(stream)
+        return e0, e1, e2, top2
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        flush.fill_(1)
+        step()
+    launch_info = mss.mss_get_last_launch()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    evs = []
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    step_ms = []
+    for _ in range(args.steps):
+        flush.fill_(1)                     # L2 flush between timed iterations (inputs are smaller than L2)
+        a, b, c, top2 = step()
+        evs.append((a, b, c))
+    barrier()
+    scan_ms = [a.elapsed_time(b) for a, b, _ in evs]
+    nw_ms = [b.elapsed_time(c) for _, b, c in evs]
+    step_ms = [a.elapsed_time(c) for a, _, c in evs]
+    total_ms = sum(step_ms)                 # device time of exactly K steps (the flush writes are outside the events)
+    clocks = sampler.stop()
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region ----------------------------------------
+    out = mss.mss_map_align_host(G, h_reads, h_mask, h_lens, m, sc, cfg.strands, 30, args.cigar_stride)   # warm-up
+    e2e_times = []
+    for _ in range(max(1, min(args.steps, 2))):
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        out = mss.mss_map_align_host(G, h_reads, h_mask, h_lens, m, sc, cfg.strands, 30, args.cigar_stride, out=out)
+        e2e_times.append(time.perf_counter() - t0)
+    e2e_s = sum(e2e_times) / len(e2e_times)
+    if dist is not None:
+        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = h_reads.numel() * 4 + h_mask.numel() * 4 + h_lens.numel() * 4
+    d2h = sum(v.numel() * v.element_size() for v in out.values())
+    same = bool((out["top2"] == top2.cpu()).all())
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peaks = measured_peaks()
+    sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_instr = n_sm * ALU_LANES_PER_CLK_SM * sm_max * 1e6              # thread-instr/s, ALU/DPX pipe at max clock
+    scan_avg_ms = sum(scan_ms) / len(scan_ms)
+    achieved = cells_step * ALGO_INSTR_PER_CELL / (scan_avg_ms * 1e-3)
+    probe_rate, _ = mss.mss_probe_dpx_peak(2048)
+    roofline = {"bound": "alu", "kernel": "scan_dpx_kernel", "achieved": achieved / 1e12, "peak": peak_instr / 1e12,
+                "unit": "T thread-instr/s", "frac": achieved / peak_instr, "traffic": None,
+                "peak_source": f"{n_sm} SMs x {ALU_LANES_PER_CLK_SM} lanes/clk x {sm_max:.0f} MHz (clocks.max.sm of MEASURED_PEAKS.json)",
+                "algorithmic_instr_per_cell": ALGO_INSTR_PER_CELL, "cells_per_launch": cells_step,
+                "kernel_ms": scan_avg_ms, "probe_dpx_peak": probe_rate / 1e12,
+                "frac_of_probe": achieved / probe_rate if probe_rate > 0 else None}
+    line = {
+        "metric": "MaxSS GCUPS (scan+top-2+NW step)", "value": cells_step * world / (ms_per_step * 1e-3) / 1e9,
+        "unit": "GCUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "s16x2 (int16 lanes, exact)",
+        "data": "synthetic",
+        "config": {"workload": f"config {cfg.c} ({cfg.name}): {n_reads} reads x {m} bp per GPU vs {cfg.genome_len} bp genome, "
+                               f"F={cfg.frag_len}, overlap={'m-1' if cfg.overlap < 0 else cfg.overlap}, both strands, top-2 + NW",
+                   "reads_per_gpu": n_reads, "read_len": m, "genome_bp": cfg.genome_len, "frag_len": cfg.frag_len,
+                   "n_frag": G.n_frag, "l2": "flushed between steps (256 MiB write); genome (1.7 MB) is L2-resident by design",
+                   "parallelism": f"reads sharded over {world} GPU(s), genome replicated, no collective",
+                   "launch": launch_info},
+        "reads_per_s": n_reads * world / (ms_per_step * 1e-3),
+        "scan_gcups": cells_step / (scan_avg_ms * 1e-3) / 1e9, "scan_ms": scan_avg_ms, "nw_ms": sum(nw_ms) / len(nw_ms),
+        "genome_load_ms": genome_load_ms,
+        "e2e": {"value": cells_step * world / e2e_s / 1e9, "unit": "GCUPS", "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s, "matches_device_path": same,
+                "api": "mss_map_align_host (pinned host buffers in/out)"},
+        "gpu_launches": args.steps * (launch_info["launches"] + (0 if args.no_nw else 1)),
+        "clocks": clocks, "roofline": roofline,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(cfg, genome, reads, lens)
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

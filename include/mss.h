@@ -157,6 +157,20 @@ int mss_map_reads_host(const mss_genome_t *g, const uint32_t *h_reads, const uin
                        mss_scoring_t sc, int32_t strands, void *d_workspace, size_t workspace_bytes,
                        void *stream, mss_top2_t *h_out);
 
+/*
+ * Both phases with HOST buffers: reads in; top-2 records, NW score, position and CIGAR out (all h_* pointers are
+ * host memory, pinned for full copy speed).  Copies in, mss_map_reads, mss_nw_align on the best hits, copies out,
+ * synchronises.  d_workspace must hold mss_map_align_host_workspace_bytes(...) bytes.
+ */
+size_t mss_map_align_host_workspace_bytes(const mss_genome_t *g, int32_t n_reads, int32_t max_len,
+                                          int32_t read_stride_words, int32_t strands, mss_scoring_t sc, int32_t pad,
+                                          int32_t cigar_stride);
+int mss_map_align_host(const mss_genome_t *g, const uint32_t *h_reads, const uint32_t *h_reads_nmask,
+                       int32_t read_stride_words, const int32_t *h_lens, int32_t n_reads, int32_t max_len,
+                       mss_scoring_t sc, int32_t strands, int32_t pad, void *d_workspace, size_t workspace_bytes,
+                       void *stream, mss_top2_t *h_top2, int32_t *h_score, int64_t *h_ref_pos, uint32_t *h_cigar,
+                       int32_t cigar_stride, int32_t *h_n_cigar);
+
 /* ---- diagnostics ------------------------------------------------------------------------------------------------ */
 
 const char *mss_strerror(int status);

@@ -72,6 +72,10 @@ def lib() -> C.CDLL:
     L.mss_map_host_workspace_bytes.argtypes = [vp, i32, i32, i32, i32]; L.mss_map_host_workspace_bytes.restype = sz
     L.mss_map_reads_host.argtypes = [vp, vp, vp, i32, vp, i32, i32, _Scoring, i32, vp, sz, vp, vp]
     L.mss_map_reads_host.restype = C.c_int
+    L.mss_map_align_host_workspace_bytes.argtypes = [vp, i32, i32, i32, i32, _Scoring, i32, i32]
+    L.mss_map_align_host_workspace_bytes.restype = sz
+    L.mss_map_align_host.argtypes = [vp, vp, vp, i32, vp, i32, i32, _Scoring, i32, i32, vp, sz, vp, vp, vp, vp, vp, i32, vp]
+    L.mss_map_align_host.restype = C.c_int
     L.mss_nw_workspace_bytes.argtypes = [vp, i32, i32, _Scoring, i32]; L.mss_nw_workspace_bytes.restype = sz
     L.mss_nw_align.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, _Scoring, i32, vp, sz, vp, vp, vp, vp, i32, vp]
     L.mss_nw_align.restype = C.c_int
@@ -195,6 +199,30 @@ def mss_map_reads_host(g: Genome, h_reads, h_reads_nmask, h_lens, max_len: int, 
     ws = g.scratch(nbytes, "maphost")
     _check(L.mss_map_reads_host(g.handle, _ptr(h_reads), _ptr(h_reads_nmask), stride, _ptr(h_lens), n, max_len, scoring.c(),
                                 strands, _ptr(ws), ws.numel(), _stream(stream), _ptr(out)), "mss_map_reads_host")
+    return out
+
+
+def mss_map_align_host(g: Genome, h_reads, h_reads_nmask, h_lens, max_len: int, scoring: Scoring = Scoring(),
+                       strands: int = MSS_BOTH, pad: int = 30, cigar_stride: int = 16, stream=None, out=None):
+    """Both phases, host (pinned) tensors in and out.  -> dict(top2, score, ref_pos, cigar, n_cigar) of host tensors."""
+    torch = _torch()
+    L = lib()
+    n = int(h_lens.numel())
+    stride = int(h_reads.shape[1])
+    if out is None:
+        out = dict(top2=torch.empty((n, 2, 4), dtype=torch.int32).pin_memory(),
+                   score=torch.empty(n, dtype=torch.int32).pin_memory(),
+                   ref_pos=torch.empty(n, dtype=torch.int64).pin_memory(),
+                   cigar=torch.empty((n, cigar_stride), dtype=torch.int32).pin_memory(),
+                   n_cigar=torch.empty(n, dtype=torch.int32).pin_memory())
+    nbytes = L.mss_map_align_host_workspace_bytes(g.handle, n, max_len, stride, strands, scoring.c(), pad, cigar_stride)
+    if nbytes == 0:
+        raise MssError(-1, "mss_map_align_host_workspace_bytes")
+    ws = g.scratch(nbytes, "e2e")
+    _check(L.mss_map_align_host(g.handle, _ptr(h_reads), _ptr(h_reads_nmask), stride, _ptr(h_lens), n, max_len, scoring.c(),
+                                strands, pad, _ptr(ws), ws.numel(), _stream(stream), _ptr(out["top2"]), _ptr(out["score"]),
+                                _ptr(out["ref_pos"]), _ptr(out["cigar"]), cigar_stride, _ptr(out["n_cigar"])),
+           "mss_map_align_host")
     return out
 
 

@@ -178,6 +178,67 @@ int mss_nw_align(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t*
     return MSS_OK;
 }
 
+namespace {
+inline size_t up256(size_t x) { return (x + 255) / 256 * 256; }
+}
+
+size_t mss_map_align_host_workspace_bytes(const mss_genome_t* g, int32_t n_reads, int32_t max_len, int32_t read_stride_words,
+                                          int32_t strands, mss_scoring_t sc, int32_t pad, int32_t cigar_stride)
+{
+    size_t a = mss_map_workspace_bytes(g, n_reads, max_len, strands);
+    size_t b = mss_nw_workspace_bytes(g, n_reads, max_len, sc, pad);
+    if (a == 0 || b == 0 || read_stride_words < 1 || cigar_stride < 1) return 0;
+    size_t n = (size_t)(n_reads > 0 ? n_reads : 1);
+    size_t scratch = up256(a > b ? a : b);
+    return scratch + up256(n * read_stride_words * 4) + up256(n * ((read_stride_words + 1) / 2) * 4) + up256(n * 4)
+         + up256(n * sizeof(mss_top2_t)) + up256(n * 4) + up256(n * 8) + up256(n * (size_t)cigar_stride * 4) + up256(n * 4);
+}
+
+int mss_map_align_host(const mss_genome_t* g, const uint32_t* h_reads, const uint32_t* h_reads_nmask, int32_t read_stride_words,
+                       const int32_t* h_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands, int32_t pad,
+                       void* d_workspace, size_t workspace_bytes, void* stream, mss_top2_t* h_top2, int32_t* h_score,
+                       int64_t* h_ref_pos, uint32_t* h_cigar, int32_t cigar_stride, int32_t* h_n_cigar)
+{
+    if (!g || n_reads < 0 || read_stride_words < 1 || cigar_stride < 1) return MSS_ERR_ARG;
+    if (n_reads == 0) return MSS_OK;
+    if (!h_reads || !h_lens || !h_top2 || !h_score || !h_ref_pos || !h_cigar || !h_n_cigar || !d_workspace) return MSS_ERR_ARG;
+    size_t need = mss_map_align_host_workspace_bytes(g, n_reads, max_len, read_stride_words, strands, sc, pad, cigar_stride);
+    if (need == 0) return MSS_ERR_ARG;
+    if (workspace_bytes < need) return MSS_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t n = (size_t)n_reads;
+    size_t a = mss_map_workspace_bytes(g, n_reads, max_len, strands), b = mss_nw_workspace_bytes(g, n_reads, max_len, sc, pad);
+    size_t scratch = up256(a > b ? a : b);
+    size_t reads_b = n * read_stride_words * 4, mask_b = n * ((read_stride_words + 1) / 2) * 4;
+    char* w = (char*)d_workspace + scratch;
+    uint32_t* d_reads = (uint32_t*)w;            w += up256(reads_b);
+    uint32_t* d_mask = (uint32_t*)w;             w += up256(mask_b);
+    int32_t* d_lens = (int32_t*)w;               w += up256(n * 4);
+    mss_top2_t* d_top2 = (mss_top2_t*)w;         w += up256(n * sizeof(mss_top2_t));
+    int32_t* d_score = (int32_t*)w;              w += up256(n * 4);
+    int64_t* d_pos = (int64_t*)w;                w += up256(n * 8);
+    uint32_t* d_cigar = (uint32_t*)w;            w += up256(n * (size_t)cigar_stride * 4);
+    int32_t* d_ncig = (int32_t*)w;
+    cudaError_t e = cudaMemcpyAsync(d_reads, h_reads, reads_b, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && h_reads_nmask) e = cudaMemcpyAsync(d_mask, h_reads_nmask, mask_b, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_lens, h_lens, n * 4, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    const uint32_t* dm = h_reads_nmask ? d_mask : nullptr;
+    int rc = mss_map_reads(g, d_reads, dm, read_stride_words, d_lens, n_reads, max_len, sc, strands, d_workspace, scratch, st, d_top2);
+    if (rc != MSS_OK) return rc;
+    rc = mss_nw_align(g, d_reads, dm, read_stride_words, d_lens, n_reads, max_len, d_top2, sc, pad, d_workspace, scratch, st,
+                      d_score, d_pos, d_cigar, cigar_stride, d_ncig);
+    if (rc != MSS_OK) return rc;
+    e = cudaMemcpyAsync(h_top2, d_top2, n * sizeof(mss_top2_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_score, d_score, n * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_ref_pos, d_pos, n * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_cigar, d_cigar, n * (size_t)cigar_stride * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h_n_cigar, d_ncig, n * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return MSS_OK;
+}
+
 int mss_mapq_filter(const mss_top2_t* d_hits, int32_t n_reads, float mapq_threshold, void* stream, uint8_t* d_mapped, float* d_mapq)
 {
     if (n_reads < 0) return MSS_ERR_ARG;

@@ -30,3 +30,16 @@ def map_reads(g, reads, lens, strands=3, match=5, mismatch=-4, variant=0, with_m
     finally:
         mss.mss_set_scan_variant(0)
     return out.cpu().numpy()
+
+
+def nw_align(g, reads, lens, top2, match=5, mismatch=-4, gap=-26, pad=30, cigar_stride=None):
+    import torch
+    import paper_1403_2136_b200 as mss
+    reads = np.asarray(reads, dtype=np.uint8)
+    lens = np.asarray(lens, dtype=np.int32)
+    rp, rn = gen.pack_reads(reads, lens)
+    sc, pos, cig, nc = mss.mss_nw_align(g, to_dev(rp), to_dev(rn), to_dev(lens), int(reads.shape[1]),
+                                        to_dev(np.ascontiguousarray(top2, dtype=np.int32)),
+                                        mss.Scoring(match, mismatch, gap), pad, cigar_stride)
+    torch.cuda.synchronize()
+    return sc.cpu().numpy(), pos.cpu().numpy(), cig.cpu().numpy().view(np.uint32), nc.cpu().numpy()
