@@ -193,6 +193,17 @@ int mss_get_last_launch(mss_launch_info_t *out);
  */
 int mss_probe_dpx_peak(int32_t iters, void *stream, double *h_instr_per_s, float *h_ms);
 
+/*
+ * Issue-rate probes behind the roofline denominator: `which` selects an instruction or mix, the result
+ * is thread-instructions (rows 11-13: cells) per clock per SM, measured with clock64 over `iters` rounds of 64 chain
+ * steps on 1024 threads per SM.  0 VIADDMNMX.S16x2.RELU, 1 VIMNMX3.S16x2, 2 their 2:1 mix, 3 PRMT, 4 LOP3, 5 IMAD,
+ * 6 HFMA2.RELU, 7 DPX+IMAD, 8 DPX+PRMT, 9 DPX+HFMA2.RELU (both counted), 10 LDS.32, 11 the scan's inner mix
+ * (LDS.32 + VIADDMNMX per 2 cells + VIMNMX3 per 4 cells), 12 PRMT + HFMA2.RELU + VIMNMX3 mix, 13 PRMT + VIADDMNMX +
+ * VIMNMX3 mix.  Synchronises the stream before returning.
+ */
+enum { MSS_PROBE_COUNT = 14 };
+int mss_probe_pipe(int32_t which, int32_t iters, void *stream, double *h_per_clk_sm);
+
 #ifdef __cplusplus
 }
 #endif

@@ -86,6 +86,7 @@ def lib() -> C.CDLL:
     L.mss_set_scan_variant.argtypes = [C.c_int]; L.mss_set_scan_variant.restype = C.c_int
     L.mss_get_last_launch.argtypes = [C.POINTER(_LaunchInfo)]; L.mss_get_last_launch.restype = C.c_int
     L.mss_probe_dpx_peak.argtypes = [i32, vp, C.POINTER(C.c_double), C.POINTER(C.c_float)]; L.mss_probe_dpx_peak.restype = C.c_int
+    L.mss_probe_pipe.argtypes = [i32, i32, vp, C.POINTER(C.c_double)]; L.mss_probe_pipe.restype = C.c_int
     _lib = L
     return L
 
@@ -275,3 +276,17 @@ def mss_probe_dpx_peak(iters: int = 4096, stream=None):
     rate, ms = C.c_double(), C.c_float()
     _check(lib().mss_probe_dpx_peak(iters, _stream(stream), C.byref(rate), C.byref(ms)), "mss_probe_dpx_peak")
     return rate.value, ms.value
+
+
+PROBE_NAMES = ["VIADDMNMX.S16x2.RELU", "VIMNMX3.S16x2", "DPX mix 2:1 (relu : max3)", "PRMT", "LOP3", "IMAD", "HFMA2.RELU",
+               "DPX + IMAD 1:1 (both counted)", "DPX + PRMT 1:1 (both counted)", "DPX + HFMA2.RELU 1:1 (both counted)",
+               "LDS.32 (conflict-free)", "scan mix: LDS.32 + VIADDMNMX /2 cells + VIMNMX3 /4 cells  [cells]",
+               "alt mix: PRMT + HFMA2.RELU /2 cells + VIMNMX3 /4 cells  [cells]",
+               "alt mix: PRMT + VIADDMNMX /2 cells + VIMNMX3 /4 cells  [cells]"]
+
+
+def mss_probe_pipe(which: int, iters: int = 2000, stream=None) -> float:
+    """-> thread-instructions (mix rows: cells) per clock per SM of probe `which` (see include/mss.h)."""
+    v = C.c_double()
+    _check(lib().mss_probe_pipe(int(which), int(iters), _stream(stream), C.byref(v)), "mss_probe_pipe")
+    return v.value

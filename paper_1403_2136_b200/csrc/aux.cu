@@ -70,3 +70,124 @@ cudaError_t run_dpx_probe(int32_t iters, cudaStream_t st, int sm_count, double* 
     cudaFree(out);
     return e == cudaSuccess ? cudaGetLastError() : e;
 }
+
+
+// ---- pipe issue-rate probes (evidence for the roofline denominator) ---------------------------------
+// Each probe runs 8 independent register chains per thread, 1024 threads x 1 block per SM, and reports
+// thread-instructions per clock per SM from clock64() around the loop.  Operands vary per thread so that nothing is
+// promoted to the uniform datapath.
+namespace {
+__device__ __forceinline__ uint32_t p_prmt(uint32_t a, uint32_t b, uint32_t s) { uint32_t d; asm volatile("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(s)); return d; }
+__device__ __forceinline__ uint32_t p_imad(uint32_t a, uint32_t b, uint32_t c) { uint32_t d; asm volatile("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c)); return d; }
+__device__ __forceinline__ uint32_t p_hfma2r(uint32_t a, uint32_t b, uint32_t c) { uint32_t d; asm volatile("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c)); return d; }
+__device__ __forceinline__ uint32_t p_lop3(uint32_t a, uint32_t b, uint32_t c) { uint32_t d; asm volatile("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(d) : "r"(a), "r"(b), "r"(c)); return d; }
+
+template <int WHICH>
+__global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long long* cyc, uint32_t a, uint32_t b, uint32_t c, int iters)
+{
+    __shared__ uint32_t sm[8192];
+    uint32_t h[8], m[8];
+    { uint32_t lz; asm volatile("mov.u32 %0, %%laneid;" : "=r"(lz)); lz >>= 5; a += lz; b += lz; c += lz; }   // opaque, per-thread
+    for (int i = threadIdx.x; i < 8192; i += blockDim.x) sm[i] = a * i;
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < 8; j++) { h[j] = a * (threadIdx.x + j + 1); m[j] = b + j + threadIdx.x * 0x00070005u; }
+    const uint32_t* myp = sm + threadIdx.x;
+    long long t0 = clock64();
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                if (WHICH == 0) h[j] = __viaddmax_s16x2_relu(h[j], m[j], c);
+                if (WHICH == 1) h[j] = __vimax3_s16x2(h[j], m[j], c);
+                if (WHICH == 2) { h[j] = __viaddmax_s16x2_relu(h[j], m[j], c); if (j & 1) m[j] = __vimax3_s16x2(m[j], h[j], h[j - 1]); }
+                if (WHICH == 3) h[j] = p_prmt(h[j], m[j], c);
+                if (WHICH == 4) h[j] = p_lop3(h[j], m[j], c);
+                if (WHICH == 5) h[j] = p_imad(h[j], m[j], c);
+                if (WHICH == 6) h[j] = p_hfma2r(h[j], m[j], c);
+                if (WHICH == 7) { h[j] = __viaddmax_s16x2_relu(h[j], b, c); m[j] = p_imad(m[j], b, c); }
+                if (WHICH == 8) { h[j] = __viaddmax_s16x2_relu(h[j], b, c); m[j] = p_prmt(m[j], b, c); }
+                if (WHICH == 9) { h[j] = __viaddmax_s16x2_relu(h[j], b, c); m[j] = p_hfma2r(m[j], b, c); }
+                if (WHICH == 10) {   // LDS.32 only (conflict-free), one LOP3 consumer each
+                    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(myp + ((u * 8 + j) & 63) * 32 + (it & 1) * 2048)));
+                    h[j] ^= v;
+                }
+                if (WHICH == 11) {   // the scan's inner mix: LDS.32 + VIADDMNMX.S16x2.RELU per 2 cells, VIMNMX3.S16x2 per 4 cells
+                    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(myp + ((u * 8 + j) & 63) * 32 + (it & 1) * 2048)));
+                    uint32_t hn = __viaddmax_s16x2_relu(h[j], v, c);
+                    if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
+                    h[j] = hn;
+                }
+                if (WHICH == 12) {   // alternative mix: PRMT table look-up + HFMA2.RELU per 2 cells, VIMNMX3.S16x2 per 4 cells
+                    uint32_t sc = p_prmt(m[j], b, h[(j + 1) & 7]);
+                    uint32_t hn = p_hfma2r(h[j], a, sc);
+                    if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
+                    h[j] = hn;
+                }
+                if (WHICH == 13) {   // alternative mix, all on the ALU pipe: PRMT + VIADDMNMX per 2 cells, VIMNMX3 per 4 cells
+                    uint32_t sc = p_prmt(m[j], b, h[(j + 1) & 7]);
+                    uint32_t hn = __viaddmax_s16x2_relu(h[j], sc, c);
+                    if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
+                    h[j] = hn;
+                }
+            }
+        }
+    }
+    long long t1 = clock64();
+    uint32_t s = 0;
+#pragma unroll
+    for (int j = 0; j < 8; j++) s ^= h[j] ^ m[j];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+    if (threadIdx.x == 0) cyc[blockIdx.x] = t1 - t0;
+}
+
+const double kProbeCount[14] = { 1, 1, 1.5, 1, 1, 1, 1, 2, 2, 2, 1, 2, 2, 2 };   // counted units per chain step (mix rows 11-13: cells)
+
+template <int WHICH>
+cudaError_t launch_pipe_probe(uint32_t* out, long long* cyc, int blocks, int iters, cudaStream_t st)
+{
+    pipe_probe_kernel<WHICH><<<blocks, 1024, 0, st>>>(out, cyc, 0x00010003u, 0x00020001u, 0u, iters);
+    return cudaGetLastError();
+}
+}  // namespace
+
+cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_count, double* per_clk_sm)
+{
+    if (which < 0 || which > 13) return cudaErrorInvalidValue;
+    uint32_t* out = nullptr; long long* cyc = nullptr;
+    int blocks = sm_count;
+    cudaError_t e = cudaMalloc(&out, (size_t)blocks * 1024 * 4);                 // probe only: not on the mapping path
+    if (e == cudaSuccess) e = cudaMalloc(&cyc, (size_t)blocks * 8);
+    if (e != cudaSuccess) { cudaFree(out); return e; }
+    for (int pass = 0; pass < 2 && e == cudaSuccess; pass++) {                   // pass 0 warms up
+        switch (which) {
+            case 0: e = launch_pipe_probe<0>(out, cyc, blocks, iters, st); break;
+            case 1: e = launch_pipe_probe<1>(out, cyc, blocks, iters, st); break;
+            case 2: e = launch_pipe_probe<2>(out, cyc, blocks, iters, st); break;
+            case 3: e = launch_pipe_probe<3>(out, cyc, blocks, iters, st); break;
+            case 4: e = launch_pipe_probe<4>(out, cyc, blocks, iters, st); break;
+            case 5: e = launch_pipe_probe<5>(out, cyc, blocks, iters, st); break;
+            case 6: e = launch_pipe_probe<6>(out, cyc, blocks, iters, st); break;
+            case 7: e = launch_pipe_probe<7>(out, cyc, blocks, iters, st); break;
+            case 8: e = launch_pipe_probe<8>(out, cyc, blocks, iters, st); break;
+            case 9: e = launch_pipe_probe<9>(out, cyc, blocks, iters, st); break;
+            case 10: e = launch_pipe_probe<10>(out, cyc, blocks, iters, st); break;
+            case 11: e = launch_pipe_probe<11>(out, cyc, blocks, iters, st); break;
+            case 12: e = launch_pipe_probe<12>(out, cyc, blocks, iters, st); break;
+            default: e = launch_pipe_probe<13>(out, cyc, blocks, iters, st); break;
+        }
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) {
+        long long* h = new long long[blocks];
+        e = cudaMemcpy(h, cyc, (size_t)blocks * 8, cudaMemcpyDeviceToHost);
+        double avg = 0;
+        for (int i = 0; i < blocks; i++) avg += (double)h[i];
+        avg /= blocks;
+        delete[] h;
+        *per_clk_sm = (double)iters * 64.0 * kProbeCount[which] * 1024.0 / avg;
+    }
+    cudaFree(out); cudaFree(cyc);
+    return e;
+}

@@ -290,4 +290,16 @@ int mss_probe_dpx_peak(int32_t iters, void* stream, double* h_instr_per_s, float
     return MSS_OK;
 }
 
+int mss_probe_pipe(int32_t which, int32_t iters, void* stream, double* h_per_clk_sm)
+{
+    if (which < 0 || which >= MSS_PROBE_COUNT || iters < 1 || !h_per_clk_sm) return MSS_ERR_ARG;
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    e = run_pipe_probe(which, iters, (cudaStream_t)stream, sms, h_per_clk_sm);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return MSS_OK;
+}
+
 }  // extern "C"

@@ -107,3 +107,4 @@ cudaError_t launch_nw(const mss_genome* g, const uint32_t* d_reads, const uint32
 
 cudaError_t launch_mapq(const mss_top2_t* d_hits, int32_t n_reads, float thr, cudaStream_t st, uint8_t* d_mapped, float* d_mapq);
 cudaError_t run_dpx_probe(int32_t iters, cudaStream_t st, int sm_count, double* instr_per_s, float* ms);
+cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_count, double* per_clk_sm);
