@@ -12,8 +12,12 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): brute force over all gap-free substring pairs, closed
  * forms (exact read = m*match, truncated prefix), reverse-complement symmetry, whole-genome = max over
  * fragments for every F, tie-break constructions, Fig. 2 fragment cutting, exhaustive
- * enumeration of all fitting alignments for NW, planted-indel CIGARs.  Nothing here is "parity unpinned".
+ * enumeration of all fitting alignments for NW, planted-indel CIGARs.  The next-row functions at the end of the file
+ * (MaxSSmap_fast, base-quality position-specific scoring) are pinned in tests/test_oracle_next_pins.py: brute force
+ * over every scored sub-range, the decimated-sequence reduction to the pinned plain scan, the uniform-score reduction
+ * to the pinned plain functions, closed-form phred values, exhaustive NW enumeration.  Nothing here is "parity unpinned".
  */
+#include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
@@ -230,5 +234,215 @@ void oracle_nw_align(const uint8_t *genome, int64_t G, int32_t F, int32_t V,
         }
         ncig_out[r] = nc;
         free(ops); free(D); free(q);
+    }
+}
+
+/* ====================================================================================================================
+ * Next rows: MaxSSmap_fast and base-quality position-specific scoring.  Same rules as above: plain
+ * loops in the paper's order, int32 arithmetic, nothing shared with the CUDA path.
+ * ==================================================================================================================== */
+
+/*
+ * MaxSSmap_fast (section 2.3): "we consider every other nucleotides in the read sequence when mapping to
+ * the genome".  Reading (reading 20): of the strand-oriented query as it is slid over the genome, only
+ * positions i = 0, 2, 4, ... are scored, each against genome position g+i as before; the maximum scoring subsequence is
+ * taken over that sub-sequence of scores.  Everything else (fragments, look-ahead, ties, top-2) is oracle_map_reads.
+ */
+static int32_t maxss_diagonal_every_other(const uint8_t *gp, int64_t g, int64_t end,
+                                          const uint8_t *r, int32_t m, const submat_t *M)
+{
+    int32_t H = 0, best = 0;
+    int32_t n = (end - g < m) ? (int32_t)(end - g) : m;
+    for (int32_t i = 0; i < n; i += 2) {
+        H += M->s[r[i]][gp[g + i]];
+        if (H < 0) H = 0;
+        if (H > best) best = H;
+    }
+    return best;
+}
+
+void oracle_map_reads_fast(const uint8_t *genome, int64_t G, int32_t F, int32_t V,
+                           const uint8_t *reads, int32_t read_stride, const int32_t *lens, int32_t n_reads,
+                           int32_t match, int32_t mismatch, int32_t strands, ohit_t *out)
+{
+    int64_t nfrag = (G + F - 1) / F;
+    int32_t max_m = 0;
+    for (int32_t r = 0; r < n_reads; r++) if (lens[r] > max_m) max_m = lens[r];
+    uint8_t *gp = padded_genome(genome, G, nfrag * F + max_m);
+    submat_t M = make_submat(match, mismatch);
+    for (int32_t r = 0; r < n_reads; r++) {
+        int32_t m = lens[r];
+        const uint8_t *fwd = reads + (int64_t)r * read_stride;
+        uint8_t *rev = (uint8_t *)malloc((size_t)(m > 0 ? m : 1));
+        reverse_complement(fwd, m, rev);
+        int32_t Veff = (V < 0 || V > m - 1) ? m - 1 : V;
+        ohit_t best = { -1, 0, 0, 0 }, second = { -1, 0, 0, 0 };
+        for (int64_t f = 0; f < nfrag; f++) {
+            int64_t end = f * F + F + Veff;
+            ohit_t fb = { (int32_t)f, 0, -1, 0 };
+            for (int32_t s = 0; s < 2; s++) {
+                if (!(strands & (1 << s))) continue;
+                const uint8_t *q = s ? rev : fwd;
+                for (int32_t d = 0; d < F; d++) {
+                    int32_t sc = maxss_diagonal_every_other(gp, f * F + d, end, q, m, &M);
+                    if (sc > fb.score) { fb.score = sc; fb.diag = d; fb.strand = s; }
+                }
+            }
+            if (best.frag < 0 || fb.score > best.score) { second = best; best = fb; }
+            else if (second.frag < 0 || fb.score > second.score) { second = fb; }
+        }
+        out[2 * r] = best;
+        out[2 * r + 1] = second;
+        free(rev);
+    }
+    free(gp);
+}
+
+/*
+ * Base qualities (section 2.2.1): "let x be the probability that the base at position i is correctly
+ * sequenced.  This can be calculated by the phred score ...  The score of a match against the nucleotide at position i
+ * is match x x and mismatch is mismatch x x/3."  Phred: Q = -10 log10(P(error)), so x = 1 - 10^(-Q/10).
+ * The paper keeps these as floats; here they are fixed-point integers (reading 22): `scale` units per score
+ * point, rounded to nearest (halves away from zero), decided in IEEE double:
+ *     pmatch[i] = round(scale*match*x_i),   pmismatch[i] = round(scale*mismatch*x_i/3).
+ */
+void oracle_pssm_from_phred(const uint8_t *qual, int64_t n, int32_t match, int32_t mismatch, int32_t scale,
+                            int32_t *pmatch, int32_t *pmismatch)
+{
+    for (int64_t i = 0; i < n; i++) {
+        double x = 1.0 - pow(10.0, -(double)qual[i] / 10.0);
+        pmatch[i] = (int32_t)llround((double)scale * (double)match * x);
+        pmismatch[i] = (int32_t)llround((double)scale * (double)mismatch * x / 3.0);
+    }
+}
+
+/* Position-specific score of read position i (already strand-oriented) against genome base b: "a position specific
+ * scoring matrix for each read".  N on either side is a mismatch (reading 6). */
+static int32_t pssm_score(uint8_t rb, uint8_t gb, int32_t pm, int32_t pmm)
+{
+    return (rb < 4 && rb == gb) ? pm : pmm;
+}
+
+/* First phase with a position-specific scoring matrix: oracle_map_reads with s(read[i], genome[g+i]) replaced by the
+ * per-position pair (pmatch[i], pmismatch[i]).  pmatch/pmismatch are rows of `read_stride` int32 per read, indexed by
+ * the position in the read as given (forward); on the reverse strand position i of the reverse-complemented read
+ * carries the scores of original position m-1-i (the quality belongs to the base call). */
+void oracle_map_reads_pssm(const uint8_t *genome, int64_t G, int32_t F, int32_t V,
+                           const uint8_t *reads, int32_t read_stride, const int32_t *lens, int32_t n_reads,
+                           const int32_t *pmatch, const int32_t *pmismatch, int32_t strands, ohit_t *out)
+{
+    int64_t nfrag = (G + F - 1) / F;
+    int32_t max_m = 0;
+    for (int32_t r = 0; r < n_reads; r++) if (lens[r] > max_m) max_m = lens[r];
+    uint8_t *gp = padded_genome(genome, G, nfrag * F + max_m);
+    for (int32_t r = 0; r < n_reads; r++) {
+        int32_t m = lens[r];
+        const uint8_t *fwd = reads + (int64_t)r * read_stride;
+        const int32_t *pm = pmatch + (int64_t)r * read_stride, *pmm = pmismatch + (int64_t)r * read_stride;
+        uint8_t *rev = (uint8_t *)malloc((size_t)(m > 0 ? m : 1));
+        int32_t *rpm = (int32_t *)malloc(sizeof(int32_t) * (size_t)(m > 0 ? m : 1));
+        int32_t *rpmm = (int32_t *)malloc(sizeof(int32_t) * (size_t)(m > 0 ? m : 1));
+        reverse_complement(fwd, m, rev);
+        for (int32_t i = 0; i < m; i++) { rpm[i] = pm[m - 1 - i]; rpmm[i] = pmm[m - 1 - i]; }
+        int32_t Veff = (V < 0 || V > m - 1) ? m - 1 : V;
+        ohit_t best = { -1, 0, 0, 0 }, second = { -1, 0, 0, 0 };
+        for (int64_t f = 0; f < nfrag; f++) {
+            int64_t end = f * F + F + Veff;
+            ohit_t fb = { (int32_t)f, 0, -1, 0 };
+            for (int32_t s = 0; s < 2; s++) {
+                if (!(strands & (1 << s))) continue;
+                const uint8_t *q = s ? rev : fwd;
+                const int32_t *qm = s ? rpm : pm, *qmm = s ? rpmm : pmm;
+                for (int32_t d = 0; d < F; d++) {
+                    int64_t g = f * F + d;
+                    int32_t n = (end - g < m) ? (int32_t)(end - g) : m;
+                    int32_t H = 0, b = 0;
+                    for (int32_t i = 0; i < n; i++) {
+                        H += pssm_score(q[i], gp[g + i], qm[i], qmm[i]);
+                        if (H < 0) H = 0;
+                        if (H > b) b = H;
+                    }
+                    if (b > fb.score) { fb.score = b; fb.diag = d; fb.strand = s; }
+                }
+            }
+            if (best.frag < 0 || fb.score > best.score) { second = best; best = fb; }
+            else if (second.frag < 0 || fb.score > second.score) { second = fb; }
+        }
+        out[2 * r] = best;
+        out[2 * r + 1] = second;
+        free(rev); free(rpm); free(rpmm);
+    }
+    free(gp);
+}
+
+/* Second phase with the same position-specific scores ("in both phases of the program"):
+ * oracle_nw_align with s(Q[i-1], W[j-1]) = pmatch/pmismatch of read position i-1 (strand-oriented as above); `gap` is
+ * given in the same fixed-point units (scale*gap).  Window, recurrence, end column, traceback order and CIGAR as in
+ * oracle_nw_align. */
+void oracle_nw_align_pssm(const uint8_t *genome, int64_t G, int32_t F, int32_t V,
+                          const uint8_t *reads, int32_t read_stride, const int32_t *lens, int32_t n_reads,
+                          const ohit_t *top2, const int32_t *pmatch, const int32_t *pmismatch, int32_t gap, int32_t pad,
+                          int32_t *score_out, int64_t *pos_out, uint32_t *cigar_out, int32_t cigar_stride, int32_t *ncig_out)
+{
+    for (int32_t r = 0; r < n_reads; r++) {
+        ohit_t h = top2[2 * r];
+        int32_t m = lens[r];
+        if (h.frag < 0) { score_out[r] = 0; pos_out[r] = -1; ncig_out[r] = 0; continue; }
+        uint8_t *q = (uint8_t *)malloc((size_t)m);
+        int32_t *qm = (int32_t *)malloc(sizeof(int32_t) * (size_t)m), *qmm = (int32_t *)malloc(sizeof(int32_t) * (size_t)m);
+        const int32_t *pm = pmatch + (int64_t)r * read_stride, *pmm = pmismatch + (int64_t)r * read_stride;
+        if (h.strand) {
+            reverse_complement(reads + (int64_t)r * read_stride, m, q);
+            for (int32_t i = 0; i < m; i++) { qm[i] = pm[m - 1 - i]; qmm[i] = pmm[m - 1 - i]; }
+        } else {
+            memcpy(q, reads + (int64_t)r * read_stride, (size_t)m);
+            for (int32_t i = 0; i < m; i++) { qm[i] = pm[i]; qmm[i] = pmm[i]; }
+        }
+        int32_t Veff = (V < 0 || V > m - 1) ? m - 1 : V;
+        int64_t ws = (int64_t)h.frag * F - pad;           if (ws < 0) ws = 0;
+        int64_t we = (int64_t)h.frag * F + F + Veff + pad; if (we > G) we = G;
+        int64_t L = we - ws, cols = L + 1;
+        int32_t *D = (int32_t *)malloc(sizeof(int32_t) * (size_t)(m + 1) * (size_t)cols);
+        for (int64_t j = 0; j <= L; j++) D[j] = 0;
+        for (int32_t i = 1; i <= m; i++) {
+            D[(int64_t)i * cols] = i * gap;
+            for (int64_t j = 1; j <= L; j++) {
+                int32_t dg = D[(int64_t)(i - 1) * cols + j - 1] + pssm_score(q[i - 1], genome[ws + j - 1], qm[i - 1], qmm[i - 1]);
+                int32_t up = D[(int64_t)(i - 1) * cols + j] + gap;
+                int32_t lf = D[(int64_t)i * cols + j - 1] + gap;
+                int32_t v = dg;
+                if (up > v) v = up;
+                if (lf > v) v = lf;
+                D[(int64_t)i * cols + j] = v;
+            }
+        }
+        int64_t jbest = 0;
+        for (int64_t j = 1; j <= L; j++)
+            if (D[(int64_t)m * cols + j] > D[(int64_t)m * cols + jbest]) jbest = j;
+        score_out[r] = D[(int64_t)m * cols + jbest];
+        uint8_t *ops = (uint8_t *)malloc((size_t)(m + L + 1));
+        int64_t nops = 0;
+        int32_t i = m; int64_t j = jbest;
+        while (i > 0) {
+            int32_t v = D[(int64_t)i * cols + j];
+            if (j > 0 && D[(int64_t)(i - 1) * cols + j - 1] + pssm_score(q[i - 1], genome[ws + j - 1], qm[i - 1], qmm[i - 1]) == v) {
+                ops[nops++] = 0; i--; j--;
+            } else if (D[(int64_t)(i - 1) * cols + j] + gap == v) {
+                ops[nops++] = 1; i--;
+            } else {
+                ops[nops++] = 2; j--;
+            }
+        }
+        pos_out[r] = ws + j;
+        int32_t nc = 0;
+        uint32_t *cg = cigar_out + (int64_t)r * cigar_stride;
+        for (int64_t k = nops - 1; k >= 0; ) {
+            uint8_t op = ops[k]; uint32_t len = 0;
+            while (k >= 0 && ops[k] == op) { len++; k--; }
+            if (nc < cigar_stride) cg[nc] = (len << 4) | op;
+            nc++;
+        }
+        ncig_out[r] = nc;
+        free(ops); free(D); free(q); free(qm); free(qmm);
     }
 }

@@ -50,6 +50,7 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
     unsigned long long* cur = (unsigned long long*)(qlen + NQ_MAX);   // NQ_MAX (per read; 8-byte aligned by layout)
     mss_hit_t* tbest = (mss_hit_t*)(cur + NQ_MAX);             // NQ_MAX
     mss_hit_t* tsecond = tbest + NQ_MAX;                       // NQ_MAX
+    int32_t* thr = (int32_t*)(tsecond + NQ_MAX);               // NQ_MAX (per read): score a fragment must exceed to matter
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int32_t group = blockIdx.x % ug.n_groups, split = blockIdx.x / ug.n_groups;
@@ -79,6 +80,7 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
         mss_hit_t none = { -1, 0, 0, 0 };
         tbest[tid] = none;
         tsecond[tid] = none;
+        thr[tid] = -1;
     }
 
     const char* my = reinterpret_cast<const char*>(planes + tid);
@@ -109,6 +111,7 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
             for (int32_t q = 0; q < nq; q++) {
                 const int32_t m = qlen[q];
                 if (m == 0) { if (lane == 0) wres[q * C::NW + warp] = 0u; continue; }
+                const int32_t need = thr[q >> (ns - 1)];       // the read's current second-best score (or -1)
                 const uint32_t* ro = roff + q * MP;
                 uint32_t H[K], B[K];
 #pragma unroll
@@ -143,6 +146,9 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
                 for (int k = 1; k < K; k++) mx = __vmaxs2(mx, B[k]);
                 uint32_t M = max(mx & 0xFFFFu, mx >> 16);
                 uint32_t W = __reduce_max_sync(0xffffffffu, M);
+                // a5 replaces only on strictly greater and fragments ascend: a fragment that does not beat the read's
+                // current second place can never enter the top-2, so its window start is not needed (slot 0 = no report)
+                if ((int32_t)W <= need) { if (lane == 0) wres[q * C::NW + warp] = 0u; continue; }
                 uint32_t d = 0xFFFFu;
                 if (M == W) {
 #pragma unroll
@@ -162,6 +168,7 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
                     if (qlen[q] == 0) continue;
                     uint32_t best = 0u;
                     for (int w = 0; w < C::NW; w++) best = max(best, wres[q * C::NW + w]);
+                    if (best == 0u) continue;                   // no warp reported (a report always has a non-zero low half)
                     int32_t strand = (ns == 2) ? s : (p.strands == 2 ? 1 : 0);
                     unsigned long long k64 = frag_key((int32_t)(best >> 16), strand, toff + (int32_t)(0xFFFFu - (best & 0xFFFFu)));
                     c = k64 > c ? k64 : c;
@@ -173,6 +180,7 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
                         mss_hit_t b = tbest[tid], s2 = tsecond[tid];
                         top2_push(b, s2, h);
                         tbest[tid] = b; tsecond[tid] = s2;
+                        thr[tid] = s2.frag >= 0 ? s2.score : -1;
                     }
                     c = 0ull;
                 }
@@ -210,7 +218,9 @@ DpxUnitGeom unit_geom(const mss_genome* g, int32_t n_reads, int32_t strands)
     ug.reads_per_group = NQ_MAX / ns;
     ug.n_groups = (n_reads + ug.reads_per_group - 1) / ug.reads_per_group;
     if (ug.n_groups < 1) ug.n_groups = 1;
-    int64_t target = (int64_t)g->sm_count * 32;
+    // blocks are long (a group of reads against a whole range of fragments): aim for >= ~48 waves of 3 resident blocks
+    // per SM so that the ragged end of the grid costs about 1 % (measured: 14 waves left ~4 % of the SMs' time idle)
+    int64_t target = (int64_t)g->sm_count * 3 * 48;
     int64_t want = (target + ug.n_groups - 1) / ug.n_groups;
     if (want < 1) want = 1;
     if (want > g->n_frag) want = g->n_frag;
@@ -230,7 +240,8 @@ cudaError_t launch_variant(const mss_genome* g, const ScanParams& p, const DpxUn
     using C = Cfg<K, T>;
     int32_t MP = (p.max_len + 3) & ~3;
     int32_t ROWW = (C::HALF + MP + 3) & ~3;
-    size_t smem = (size_t)(5 * ROWW + NQ_MAX * MP + NQ_MAX * C::NW) * 4 + NQ_MAX * 4 + NQ_MAX * 8 + 2 * NQ_MAX * sizeof(mss_hit_t);
+    size_t smem = (size_t)(5 * ROWW + NQ_MAX * MP + NQ_MAX * C::NW) * 4 + NQ_MAX * 4 + NQ_MAX * 8 + 2 * NQ_MAX * sizeof(mss_hit_t)
+                + NQ_MAX * 4;
     if (smem > (size_t)g->max_smem_optin) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(scan_dpx_kernel<K, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
