@@ -8,7 +8,7 @@ stated in DESIGN.md section 4 and the 2-bit / N-mask wire format of include/mss.
 from .synth import (  # noqa: F401
     A, C, G, T, N, S0,
     Config, CONFIGS, config,
-    make_genome, make_reads, revcomp,
+    make_genome, make_reads, make_quals, revcomp,
     pack_2bit, unpack_2bit, pack_reads, sha256_of,
     decode, encode,
 )

@@ -247,6 +247,24 @@ def make_reads(genome: np.ndarray, n_reads: int, m: int, seed: int, *,
                 strand=strand, span=span.astype(np.int32), p=p, n_indel=k.astype(np.int32))
 
 
+def make_quals(n_reads: int, m: int, seed: int) -> np.ndarray:
+    """Synthetic phred base qualities, uint8 (n_reads, m), in read order (stands in for the real MiSeq qualities the
+    paper's simulated reads carry).  Illumina-like shape: a per-read level ~ N(36, 3), a decline of
+    0..14 towards the 3' end (linear in the position, slope drawn per read), per-base noise N(0, 3), values clipped
+    to [2, 41]; with probability 0.15 the last U{1..m//4} bases are a Q2 tail (the "B-tail" of old Illumina runs)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    level = rng.normal(36.0, 3.0, size=(n_reads, 1))
+    drop = rng.uniform(0.0, 14.0, size=(n_reads, 1))
+    pos = np.arange(m, dtype=np.float64)[None, :] / max(m - 1, 1)
+    q = level - drop * pos + rng.normal(0.0, 3.0, size=(n_reads, m))
+    q = np.clip(np.rint(q), 2, 41).astype(np.uint8)
+    tail = rng.random(n_reads) < 0.15
+    tl = rng.integers(1, max(2, m // 4 + 1), size=n_reads)
+    cut = (np.arange(m)[None, :] >= (m - tl)[:, None]) & tail[:, None]
+    q[cut] = 2
+    return np.ascontiguousarray(q)
+
+
 # ----------------------------------------------------------------------------- the five configs
 
 @dataclass(frozen=True)

@@ -13,6 +13,8 @@
  *   mss_nw_align      PAPER.md:59, :91: "we align the read sequence with Needleman-Wunsch to the genome region from
  *                     the first part", match 5, mismatch -4, gap -26.
  *   mss_mapq_filter   PAPER.md:57, :63: mapped iff second/best < 0.9; MAPQ = -100 log2(second/best).
+ *   mss_map_reads_fast   PAPER.md:93: MaxSSmap_fast, every other read nucleotide.
+ *   mss_pssm_build, mss_map_reads_pssm, mss_nw_align_pssm   PAPER.md:61: base-quality position-specific scoring.
  *
  * Conventions
  *   - Every pointer named d_* is DEVICE memory owned by the caller; h_* is HOST memory owned by the caller.
@@ -142,6 +144,57 @@ int mss_nw_align(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t 
  */
 int mss_mapq_filter(const mss_top2_t *d_hits, int32_t n_reads, float mapq_threshold,
                     void *stream, uint8_t *d_mapped, float *d_mapq);
+
+/* ---- next rows: MaxSSmap_fast and base-quality position-specific scoring ------------------------------------------- */
+
+/*
+ * MaxSSmap_fast (section 2.3): "we consider every other nucleotides in the read sequence when mapping to
+ * the genome".  Same arguments, output and errors as mss_map_reads; of the strand-oriented read only positions
+ * i = 0, 2, 4, ... are scored (each still against genome[f*F+d+i]) and the maximum scoring subsequence is taken over
+ * that sub-sequence of scores (reading 20).  Workspace: mss_map_workspace_bytes.
+ */
+int mss_map_reads_fast(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
+                       int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
+                       mss_scoring_t sc, int32_t strands, void *d_workspace, size_t workspace_bytes,
+                       void *stream, mss_top2_t *d_out);
+
+/*
+ * Position-specific scoring matrix from base qualities (section 2.2.1): "let x be the probability that
+ * the base at position i is correctly sequenced ... The score of a match against the nucleotide at position i is
+ * match x x and mismatch is mismatch x x/3."  x = 1 - 10^(-Q/10) for phred quality Q.  The paper keeps floats; here
+ * the table is fixed point with `scale` units per score point (reading 22):
+ *     pmatch = round(scale*match*x), pmismatch = round(scale*mismatch*x/3)   (IEEE double, halves away from zero)
+ *   d_qual             phred values (0..93; larger values count as 93), rows of qual_stride bytes, read order
+ *   d_pssm             out: rows of pssm_stride uint32 per read, entry i = (uint16)pmatch_i | (uint16)pmismatch_i << 16
+ *                      (two int16); entries at or beyond len[r] are 0
+ *   scale >= 1         scale*match <= 32767, scale*mismatch >= -32768, else MSS_ERR_RANGE
+ * A caller may also fill d_pssm itself with any table satisfying pmismatch_i <= 0 <= pmatch_i.
+ */
+int mss_pssm_build(const uint8_t *d_qual, int32_t qual_stride, const int32_t *d_lens, int32_t n_reads,
+                   mss_scoring_t sc, int32_t scale, void *stream, uint32_t *d_pssm, int32_t pssm_stride);
+
+/*
+ * mss_map_reads with s(read[i], genome base) replaced by the read's own table: pmatch_i if the bases are equal (and
+ * neither is N) else pmismatch_i; on the reverse strand position i of the reverse-complemented read carries the
+ * entry of original position len-1-i.  `bound` states the table's range for the 16-bit lane check:
+ * bound.match >= every pmatch_i, bound.mismatch <= every pmismatch_i (for a table from mss_pssm_build:
+ * {scale*match, scale*mismatch, scale*gap}); max_len*bound.match <= 32767 else MSS_ERR_RANGE; entries outside the
+ * stated bound give undefined scores.  pssm_stride >= max_len.  Workspace: mss_map_workspace_bytes.
+ */
+int mss_map_reads_pssm(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
+                       int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
+                       const uint32_t *d_pssm, int32_t pssm_stride, mss_scoring_t bound, int32_t strands,
+                       void *d_workspace, size_t workspace_bytes, void *stream, mss_top2_t *d_out);
+
+/*
+ * mss_nw_align with the same per-position scores ("in both phases of the program"); bound.gap is the
+ * gap cost in the table's units (scale*gap).  Workspace: mss_nw_workspace_bytes(g, n_reads, max_len, bound, pad).
+ */
+int mss_nw_align_pssm(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
+                      int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
+                      const mss_top2_t *d_hits, const uint32_t *d_pssm, int32_t pssm_stride, mss_scoring_t bound,
+                      int32_t pad, void *d_workspace, size_t workspace_bytes, void *stream,
+                      int32_t *d_score, int64_t *d_ref_pos, uint32_t *d_cigar, int32_t cigar_stride, int32_t *d_n_cigar);
 
 /* ---- end-to-end convenience with HOST buffers (used for the e2e timing of bench.py) ---------------------------- */
 

@@ -80,6 +80,12 @@ def lib() -> C.CDLL:
     L.mss_nw_align.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, _Scoring, i32, vp, sz, vp, vp, vp, vp, i32, vp]
     L.mss_nw_align.restype = C.c_int
     L.mss_mapq_filter.argtypes = [vp, i32, C.c_float, vp, vp, vp]; L.mss_mapq_filter.restype = C.c_int
+    L.mss_map_reads_fast.argtypes = L.mss_map_reads.argtypes; L.mss_map_reads_fast.restype = C.c_int
+    L.mss_pssm_build.argtypes = [vp, i32, vp, i32, _Scoring, i32, vp, vp, i32]; L.mss_pssm_build.restype = C.c_int
+    L.mss_map_reads_pssm.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, i32, _Scoring, i32, vp, sz, vp, vp]
+    L.mss_map_reads_pssm.restype = C.c_int
+    L.mss_nw_align_pssm.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, vp, i32, _Scoring, i32, vp, sz, vp, vp, vp, vp, i32, vp]
+    L.mss_nw_align_pssm.restype = C.c_int
     L.mss_strerror.argtypes = [C.c_int]; L.mss_strerror.restype = C.c_char_p
     L.mss_last_cuda_error.argtypes = []; L.mss_last_cuda_error.restype = C.c_int
     L.mss_version.argtypes = []; L.mss_version.restype = C.c_int
@@ -183,6 +189,84 @@ def mss_map_reads(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, scori
     _check(L.mss_map_reads(g.handle, _ptr(d_reads), _ptr(d_reads_nmask), stride, _ptr(d_lens), n, max_len, scoring.c(),
                            strands, _ptr(ws), ws.numel(), _stream(stream), _ptr(out)), "mss_map_reads")
     return out
+
+
+def mss_map_reads_fast(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, scoring: Scoring = Scoring(),
+                       strands: int = MSS_BOTH, stream=None, out=None):
+    """MaxSSmap_fast: as mss_map_reads, scoring every other read nucleotide."""
+    torch = _torch()
+    L = lib()
+    n = int(d_lens.numel())
+    stride = int(d_reads.shape[1]) if d_reads.dim() == 2 else int(d_reads.numel() // max(n, 1))
+    if out is None:
+        out = torch.empty((n, 2, 4), dtype=torch.int32, device=d_lens.device)
+    nbytes = L.mss_map_workspace_bytes(g.handle, n, max_len, strands)
+    if nbytes == 0:
+        raise MssError(-1, "mss_map_workspace_bytes")
+    ws = g.scratch(nbytes, "map")
+    _check(L.mss_map_reads_fast(g.handle, _ptr(d_reads), _ptr(d_reads_nmask), stride, _ptr(d_lens), n, max_len, scoring.c(),
+                                strands, _ptr(ws), ws.numel(), _stream(stream), _ptr(out)), "mss_map_reads_fast")
+    return out
+
+
+def pssm_bound(scoring: Scoring, scale: int) -> Scoring:
+    """The range of a table built by mss_pssm_build(scoring, scale): {scale*match, scale*mismatch, scale*gap}."""
+    return Scoring(scale * scoring.match, scale * scoring.mismatch, scale * scoring.gap)
+
+
+def mss_pssm_build(d_qual, d_lens, scoring: Scoring = Scoring(), scale: int = 16, pssm_stride: int | None = None, stream=None):
+    """phred qualities (CUDA uint8 tensor (n, qual_stride)) -> CUDA int32 tensor (n, pssm_stride) of packed
+    (int16 pmatch | int16 pmismatch << 16) entries."""
+    torch = _torch()
+    n = int(d_lens.numel())
+    qs = int(d_qual.shape[1])
+    ps = pssm_stride or qs
+    out = torch.empty((n, ps), dtype=torch.int32, device=d_lens.device)
+    _check(lib().mss_pssm_build(_ptr(d_qual), qs, _ptr(d_lens), n, scoring.c(), int(scale), _stream(stream), _ptr(out), ps),
+           "mss_pssm_build")
+    return out
+
+
+def mss_map_reads_pssm(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, d_pssm, bound: Scoring,
+                       strands: int = MSS_BOTH, stream=None, out=None):
+    """mss_map_reads with per-read position-specific scores (d_pssm from mss_pssm_build; bound = pssm_bound(...))."""
+    torch = _torch()
+    L = lib()
+    n = int(d_lens.numel())
+    stride = int(d_reads.shape[1])
+    if out is None:
+        out = torch.empty((n, 2, 4), dtype=torch.int32, device=d_lens.device)
+    nbytes = L.mss_map_workspace_bytes(g.handle, n, max_len, strands)
+    if nbytes == 0:
+        raise MssError(-1, "mss_map_workspace_bytes")
+    ws = g.scratch(nbytes, "map")
+    _check(L.mss_map_reads_pssm(g.handle, _ptr(d_reads), _ptr(d_reads_nmask), stride, _ptr(d_lens), n, max_len, _ptr(d_pssm),
+                                int(d_pssm.shape[1]), bound.c(), strands, _ptr(ws), ws.numel(), _stream(stream), _ptr(out)),
+           "mss_map_reads_pssm")
+    return out
+
+
+def mss_nw_align_pssm(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, d_hits, d_pssm, bound: Scoring, pad: int = 30,
+                      cigar_stride: int | None = None, stream=None):
+    """mss_nw_align with per-read position-specific scores; bound.gap = the gap cost in the table's units."""
+    torch = _torch()
+    L = lib()
+    n = int(d_lens.numel())
+    stride = int(d_reads.shape[1])
+    cs = cigar_stride or (2 * max_len + 1)
+    dev = d_lens.device
+    score = torch.empty(n, dtype=torch.int32, device=dev)
+    pos = torch.empty(n, dtype=torch.int64, device=dev)
+    cigar = torch.zeros((n, cs), dtype=torch.int32, device=dev)
+    ncig = torch.empty(n, dtype=torch.int32, device=dev)
+    nbytes = L.mss_nw_workspace_bytes(g.handle, n, max_len, bound.c(), pad)
+    if nbytes == 0:
+        raise MssError(-1, "mss_nw_workspace_bytes")
+    ws = g.scratch(nbytes, "nw")
+    _check(L.mss_nw_align_pssm(g.handle, _ptr(d_reads), _ptr(d_reads_nmask), stride, _ptr(d_lens), n, max_len, _ptr(d_hits),
+                               _ptr(d_pssm), int(d_pssm.shape[1]), bound.c(), pad, _ptr(ws), ws.numel(), _stream(stream),
+                               _ptr(score), _ptr(pos), _ptr(cigar), cs, _ptr(ncig)), "mss_nw_align_pssm")
+    return score, pos, cigar, ncig
 
 
 def mss_map_reads_host(g: Genome, h_reads, h_reads_nmask, h_lens, max_len: int, scoring: Scoring = Scoring(),

@@ -26,6 +26,30 @@ cudaError_t launch_mapq(const mss_top2_t* d_hits, int32_t n_reads, float thr, cu
     return cudaGetLastError();
 }
 
+// Base qualities -> per-position (pmatch, pmismatch) table rows: a 94-entry lookup of the phred value
+// (values above 93, the FASTQ maximum, count as 93); positions at or beyond len[r] get (0, 0).
+__global__ void pssm_build_kernel(const uint8_t* __restrict__ qual, int32_t qual_stride, const int32_t* __restrict__ lens,
+                                  int32_t n_reads, PssmLut lut, uint32_t* __restrict__ pssm, int32_t pssm_stride)
+{
+    int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (int64_t)n_reads * pssm_stride) return;
+    int32_t r = (int32_t)(idx / pssm_stride), i = (int32_t)(idx % pssm_stride);
+    uint32_t v = 0u;
+    if (i < lens[r] && i < qual_stride) {
+        uint32_t q = qual[(int64_t)r * qual_stride + i];
+        v = lut.v[q > 93u ? 93u : q];
+    }
+    pssm[idx] = v;
+}
+
+cudaError_t launch_pssm_build(const uint8_t* d_qual, int32_t qual_stride, const int32_t* d_lens, int32_t n_reads,
+                              const PssmLut& lut, cudaStream_t st, uint32_t* d_pssm, int32_t pssm_stride)
+{
+    int64_t total = (int64_t)n_reads * pssm_stride;
+    pssm_build_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(d_qual, qual_stride, d_lens, n_reads, lut, d_pssm, pssm_stride);
+    return cudaGetLastError();
+}
+
 // 8 independent chains per thread, per round: 8 VIADDMNMX.S16x2.RELU + 4 VIMNMX3.S16x2 (the scan's own 2:1 mix)
 __global__ void __launch_bounds__(1024) dpx_probe_kernel(uint32_t* out, uint32_t a, uint32_t b, int iters)
 {

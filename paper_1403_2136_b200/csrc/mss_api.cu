@@ -1,4 +1,5 @@
 // C ABI of include/mss.h: argument checks, handle, variant dispatch.  No compute lives here.
+#include <cmath>
 #include <new>
 #include "mss_common.cuh"
 
@@ -83,9 +84,10 @@ size_t mss_map_workspace_bytes(const mss_genome_t* g, int32_t n_reads, int32_t m
     return a > b ? a : b;
 }
 
-int mss_map_reads(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
-                  const int32_t* d_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands,
-                  void* d_workspace, size_t workspace_bytes, void* stream, mss_top2_t* d_out)
+static int map_reads_impl(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                          const int32_t* d_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands,
+                          void* d_workspace, size_t workspace_bytes, void* stream, mss_top2_t* d_out,
+                          int32_t istep, const uint32_t* d_pssm, int32_t pssm_stride)
 {
     if (!g || n_reads < 0 || strands < 1 || strands > 3 || max_len < 1) return MSS_ERR_ARG;
     if (n_reads == 0) return MSS_OK;
@@ -99,12 +101,61 @@ int mss_map_reads(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t
     p.F = g->frag_len; p.V = g->overlap; p.n_frag = g->n_frag;
     p.reads = d_reads; p.reads_nmask = d_reads_nmask; p.stride_words = read_stride_words; p.lens = d_lens;
     p.n_reads = n_reads; p.max_len = max_len; p.match = sc.match; p.mismatch = sc.mismatch; p.strands = strands; p.zero = 0;
+    p.istep = istep; p.pssm = d_pssm; p.pssm_stride = pssm_stride;
     cudaError_t e;
     bool use_generic = (t_variant == 1) || !scan_dpx_supported(g, p);
     if (use_generic) e = launch_scan_generic(g, p, d_workspace, workspace_bytes, d_out, (cudaStream_t)stream, &t_info);
     else e = launch_scan_dpx(g, p, d_workspace, workspace_bytes, d_out, (cudaStream_t)stream, &t_info, t_variant);
     if (e != cudaSuccess) return cuda_fail(e);
     return MSS_OK;
+}
+
+int mss_map_reads(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                  const int32_t* d_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands,
+                  void* d_workspace, size_t workspace_bytes, void* stream, mss_top2_t* d_out)
+{
+    return map_reads_impl(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, sc, strands, d_workspace,
+                          workspace_bytes, stream, d_out, 1, nullptr, 0);
+}
+
+int mss_map_reads_fast(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                       const int32_t* d_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands,
+                       void* d_workspace, size_t workspace_bytes, void* stream, mss_top2_t* d_out)
+{
+    return map_reads_impl(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, sc, strands, d_workspace,
+                          workspace_bytes, stream, d_out, 2, nullptr, 0);
+}
+
+int mss_pssm_build(const uint8_t* d_qual, int32_t qual_stride, const int32_t* d_lens, int32_t n_reads, mss_scoring_t sc,
+                   int32_t scale, void* stream, uint32_t* d_pssm, int32_t pssm_stride)
+{
+    if (n_reads < 0 || qual_stride < 1 || pssm_stride < 1 || scale < 1) return MSS_ERR_ARG;
+    if (n_reads == 0) return MSS_OK;
+    if (!d_qual || !d_lens || !d_pssm) return MSS_ERR_ARG;
+    if (sc.match <= 0 || sc.mismatch >= 0) return MSS_ERR_RANGE;
+    if ((int64_t)scale * sc.match > 32767 || (int64_t)scale * sc.mismatch < -32768) return MSS_ERR_RANGE;
+    // phred Q -> x = P(base correct) = 1 - 10^(-Q/10); match*x and mismatch*x/3 in fixed point, decided
+    // in IEEE double on the host (94 values), rounded to nearest with halves away from zero
+    PssmLut lut;
+    for (int q = 0; q < 94; q++) {
+        double x = 1.0 - pow(10.0, -(double)q / 10.0);
+        long long pm = llround((double)scale * (double)sc.match * x);
+        long long px = llround((double)scale * (double)sc.mismatch * x / 3.0);
+        lut.v[q] = ((uint32_t)(uint16_t)(int16_t)pm) | ((uint32_t)(uint16_t)(int16_t)px << 16);
+    }
+    cudaError_t e = launch_pssm_build(d_qual, qual_stride, d_lens, n_reads, lut, (cudaStream_t)stream, d_pssm, pssm_stride);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return MSS_OK;
+}
+
+int mss_map_reads_pssm(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                       const int32_t* d_lens, int32_t n_reads, int32_t max_len, const uint32_t* d_pssm, int32_t pssm_stride,
+                       mss_scoring_t bound, int32_t strands, void* d_workspace, size_t workspace_bytes, void* stream,
+                       mss_top2_t* d_out)
+{
+    if (n_reads > 0 && (!d_pssm || pssm_stride < max_len)) return MSS_ERR_ARG;
+    return map_reads_impl(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, bound, strands, d_workspace,
+                          workspace_bytes, stream, d_out, 1, d_pssm, pssm_stride);
 }
 
 size_t mss_map_host_workspace_bytes(const mss_genome_t* g, int32_t n_reads, int32_t max_len, int32_t read_stride_words,
@@ -158,10 +209,11 @@ size_t mss_nw_workspace_bytes(const mss_genome_t* g, int32_t n_reads, int32_t ma
     return nw_workspace(g, n_reads, max_len, sc, pad);
 }
 
-int mss_nw_align(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+static int nw_align_impl(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
                  const int32_t* d_lens, int32_t n_reads, int32_t max_len, const mss_top2_t* d_hits, mss_scoring_t sc,
                  int32_t pad, void* d_workspace, size_t workspace_bytes, void* stream,
-                 int32_t* d_score, int64_t* d_ref_pos, uint32_t* d_cigar, int32_t cigar_stride, int32_t* d_n_cigar)
+                 int32_t* d_score, int64_t* d_ref_pos, uint32_t* d_cigar, int32_t cigar_stride, int32_t* d_n_cigar,
+                 const uint32_t* d_pssm, int32_t pssm_stride)
 {
     if (!g || n_reads < 0 || max_len < 1 || pad < 0 || cigar_stride < 1) return MSS_ERR_ARG;
     if (n_reads == 0) return MSS_OK;
@@ -171,11 +223,31 @@ int mss_nw_align(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t*
     if (max_len > MSS_MAX_READ_LEN) return MSS_ERR_RANGE;
     if ((int64_t)max_len * (int64_t)(-sc.gap) > (1ll << 30) || (int64_t)max_len * sc.match > (1ll << 30)) return MSS_ERR_RANGE;
     if (workspace_bytes < mss_nw_workspace_bytes(g, n_reads, max_len, sc, pad)) return MSS_ERR_WORKSPACE;
-    cudaError_t e = launch_nw(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, d_hits, sc, pad,
-                              d_workspace, workspace_bytes, (cudaStream_t)stream, d_score, d_ref_pos, d_cigar, cigar_stride,
-                              d_n_cigar);
+    cudaError_t e = launch_nw(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, d_hits, d_pssm, pssm_stride,
+                              sc, pad, d_workspace, workspace_bytes, (cudaStream_t)stream, d_score, d_ref_pos, d_cigar,
+                              cigar_stride, d_n_cigar);
     if (e != cudaSuccess) return cuda_fail(e);
     return MSS_OK;
+}
+
+int mss_nw_align(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                 const int32_t* d_lens, int32_t n_reads, int32_t max_len, const mss_top2_t* d_hits, mss_scoring_t sc,
+                 int32_t pad, void* d_workspace, size_t workspace_bytes, void* stream,
+                 int32_t* d_score, int64_t* d_ref_pos, uint32_t* d_cigar, int32_t cigar_stride, int32_t* d_n_cigar)
+{
+    return nw_align_impl(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, d_hits, sc, pad, d_workspace,
+                         workspace_bytes, stream, d_score, d_ref_pos, d_cigar, cigar_stride, d_n_cigar, nullptr, 0);
+}
+
+int mss_nw_align_pssm(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                      const int32_t* d_lens, int32_t n_reads, int32_t max_len, const mss_top2_t* d_hits,
+                      const uint32_t* d_pssm, int32_t pssm_stride, mss_scoring_t bound, int32_t pad,
+                      void* d_workspace, size_t workspace_bytes, void* stream,
+                      int32_t* d_score, int64_t* d_ref_pos, uint32_t* d_cigar, int32_t cigar_stride, int32_t* d_n_cigar)
+{
+    if (n_reads > 0 && (!d_pssm || pssm_stride < max_len)) return MSS_ERR_ARG;
+    return nw_align_impl(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, d_hits, bound, pad, d_workspace,
+                         workspace_bytes, stream, d_score, d_ref_pos, d_cigar, cigar_stride, d_n_cigar, d_pssm, pssm_stride);
 }
 
 namespace {

@@ -35,6 +35,9 @@ struct ScanParams {
     int32_t match, mismatch;
     int32_t strands;               // MSS_FWD | MSS_REV
     int32_t zero;                  // always 0; a run-time zero the compiler cannot fold (DPX third operand)
+    int32_t istep;                 // 1 = every read position; 2 = MaxSSmap_fast, every other position
+    const uint32_t* pssm;          // nullable: per-read rows of (int16 pmatch | int16 pmismatch << 16) per position
+    int32_t pssm_stride;           // words per row of pssm
 };
 
 // candidate of one fragment for one read: higher key = better under (score desc, strand asc, diag asc)
@@ -96,15 +99,25 @@ cudaError_t launch_scan_generic(const mss_genome* g, const ScanParams& p, void* 
 
 size_t scan_dpx_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, int32_t strands);
 bool scan_dpx_supported(const mss_genome* g, const ScanParams& p);
+// per-position (pmatch, pmismatch) of the strand-oriented query: position i of the reverse-complemented read carries the
+// scores of original position m-1-i (the quality belongs to the base call)
+__device__ __forceinline__ uint32_t pssm_at(const uint32_t* row, int32_t m, int32_t i, int32_t strand)
+{
+    return row[strand ? (m - 1 - i) : i];
+}
 cudaError_t launch_scan_dpx(const mss_genome* g, const ScanParams& p, void* ws, size_t ws_bytes,
                             mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info, int variant);
 
 size_t nw_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t pad);
 cudaError_t launch_nw(const mss_genome* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t stride_words,
                       const int32_t* d_lens, int32_t n_reads, int32_t max_len, const mss_top2_t* d_hits,
+                      const uint32_t* d_pssm, int32_t pssm_stride,
                       mss_scoring_t sc, int32_t pad, void* ws, size_t ws_bytes, cudaStream_t st,
                       int32_t* d_score, int64_t* d_ref_pos, uint32_t* d_cigar, int32_t cigar_stride, int32_t* d_n_cigar);
 
+struct PssmLut { uint32_t v[94]; };   // phred 0..93 -> packed (pmatch, pmismatch), computed on the host in double
+cudaError_t launch_pssm_build(const uint8_t* d_qual, int32_t qual_stride, const int32_t* d_lens, int32_t n_reads,
+                              const PssmLut& lut, cudaStream_t st, uint32_t* d_pssm, int32_t pssm_stride);
 cudaError_t launch_mapq(const mss_top2_t* d_hits, int32_t n_reads, float thr, cudaStream_t st, uint8_t* d_mapped, float* d_mapq);
 cudaError_t run_dpx_probe(int32_t iters, cudaStream_t st, int sm_count, double* instr_per_s, float* ms);
 cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_count, double* per_clk_sm);

@@ -23,6 +23,7 @@ struct NwParams {
     const uint32_t* gpacked; const uint32_t* gnmask; int64_t n_bases; int32_t F, V;
     const uint32_t* reads; const uint32_t* reads_nmask; int32_t stride_words; const int32_t* lens; int32_t n_reads, max_len;
     const mss_top2_t* hits; int32_t match, mismatch, gap, pad;
+    const uint32_t* pssm; int32_t pssm_stride;  // nullable: per-position (pmatch, pmismatch) rows ("both phases")
     int32_t* score; int64_t* ref_pos; uint32_t* cigar; int32_t cigar_stride; int32_t* n_cigar;
     // workspace, per warp slot
     int32_t* bnd; int64_t bnd_stride;          // boundary row between bands
@@ -34,7 +35,8 @@ struct NwParams {
 // One band of the systolic recurrence over window columns (c0, c0+ncols] (c0 = the column treated as column 0).
 // Returns through best/jbest the running (max, smallest column) of row m when this band holds it.
 template <int RB, bool TRACE>
-__device__ __forceinline__ void nw_band(const NwParams& p, const uint32_t* q /*RB codes of this lane*/, int32_t row0 /*rows above this lane's strip*/,
+__device__ __forceinline__ void nw_band(const NwParams& p, const uint32_t* q /*RB codes of this lane*/,
+                                        const int32_t* qm /*RB match scores*/, const int32_t* qx /*RB mismatch scores*/, int32_t row0 /*rows above this lane's strip*/,
                                         bool first_band, bool last_band_store, int64_t wstart /*genome position of column c0+1*/,
                                         int32_t ncols, int32_t* bnd, uint32_t* tb_band, uint8_t* wbuf,
                                         int32_t lm, int32_t rm, bool holds_m, int32_t& best, int32_t& jbest, int32_t m)
@@ -71,8 +73,7 @@ __device__ __forceinline__ void nw_band(const NwParams& p, const uint32_t* q /*R
                 uint32_t dirs = 0;
 #pragma unroll
                 for (int r = 0; r < RB; r++) {
-                    int32_t s = (q[r] == wb) ? p.match : p.mismatch;      // q[r] = 4 (N / beyond the read) never equals wb < 4; wb = 4 never matches q < 4 ... and 4 == 4 must not match:
-                    if (wb >= 4u) s = p.mismatch;
+                    int32_t s = (q[r] == wb && wb < 4u) ? qm[r] : qx[r];   // N on either side (code 4) is a mismatch
                     int32_t a = dg + s, b = up + p.gap, c = Dl[r] + p.gap;
                     int32_t v = max(a, max(b, c));
                     if (TRACE) dirs |= (a == v ? 0u : (b == v ? 1u : 2u)) << (2 * r);
@@ -117,6 +118,7 @@ nw_kernel(NwParams p, int32_t n_slots)
         }
         const uint32_t* rw = p.reads + (int64_t)r * p.stride_words;
         const uint32_t* rn = p.reads_nmask ? p.reads_nmask + (int64_t)r * ((p.stride_words + 1) / 2) : nullptr;
+        const uint32_t* prow = p.pssm ? p.pssm + (int64_t)r * p.pssm_stride : nullptr;
         const int32_t veff = (p.V < 0 || p.V > m - 1) ? m - 1 : p.V;
         int64_t ws = (int64_t)h.frag * p.F - p.pad; if (ws < 0) ws = 0;
         int64_t we = (int64_t)h.frag * p.F + p.F + veff + p.pad; if (we > p.n_bases) we = p.n_bases;
@@ -127,15 +129,20 @@ nw_kernel(NwParams p, int32_t n_slots)
         // ---- pass 1: score and end column -------------------------------------------------------------------------
         int32_t best = 0, jbest = 0;
         for (int32_t b = 0; b < nbands; b++) {
-            uint32_t q[RB];
+            uint32_t q[RB]; int32_t qm[RB], qx[RB];
 #pragma unroll
             for (int k = 0; k < RB; k++) {
                 int32_t i = b * BAND + lane * RB + k;                  // 0-based read position
                 q[k] = (i < m) ? read_base(rw, rn, m, i, h.strand) : 4u;
+                qm[k] = p.match; qx[k] = p.mismatch;
+                if (prow && i < m) {
+                    uint32_t w = pssm_at(prow, m, i, h.strand);
+                    qm[k] = (int32_t)(int16_t)(w & 0xFFFFu); qx[k] = (int32_t)(int16_t)(w >> 16);
+                }
             }
             if (b > 0 && lane == 0) bnd[0] = b * BAND * p.gap;
             __syncwarp();
-            nw_band<RB, false>(p, q, b * BAND + lane * RB, b == 0, b + 1 < nbands, ws, L, bnd, nullptr, wbuf,
+            nw_band<RB, false>(p, q, qm, qx, b * BAND + lane * RB, b == 0, b + 1 < nbands, ws, L, bnd, nullptr, wbuf,
                                lm, rm, b == bm, best, jbest, m);
             __syncwarp();
         }
@@ -150,15 +157,20 @@ nw_kernel(NwParams p, int32_t n_slots)
         const int32_t Lb = jbest - jlo;
         int32_t best2 = 0, jbest2 = 0;
         for (int32_t b = 0; b < nbands; b++) {
-            uint32_t q[RB];
+            uint32_t q[RB]; int32_t qm[RB], qx[RB];
 #pragma unroll
             for (int k = 0; k < RB; k++) {
                 int32_t i = b * BAND + lane * RB + k;
                 q[k] = (i < m) ? read_base(rw, rn, m, i, h.strand) : 4u;
+                qm[k] = p.match; qx[k] = p.mismatch;
+                if (prow && i < m) {
+                    uint32_t w = pssm_at(prow, m, i, h.strand);
+                    qm[k] = (int32_t)(int16_t)(w & 0xFFFFu); qx[k] = (int32_t)(int16_t)(w >> 16);
+                }
             }
             if (b > 0 && lane == 0) bnd[0] = b * BAND * p.gap;
             __syncwarp();
-            nw_band<RB, true>(p, q, b * BAND + lane * RB, b == 0, b + 1 < nbands, ws + jlo, Lb, bnd,
+            nw_band<RB, true>(p, q, qm, qx, b * BAND + lane * RB, b == 0, b + 1 < nbands, ws + jlo, Lb, bnd,
                               tb + (int64_t)b * p.wmax * 32, wbuf, lm, rm, b == bm, best2, jbest2, m);
             __syncwarp();
         }
@@ -239,6 +251,7 @@ size_t nw_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, mss_s
 
 cudaError_t launch_nw(const mss_genome* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t stride_words,
                       const int32_t* d_lens, int32_t n_reads, int32_t max_len, const mss_top2_t* d_hits,
+                      const uint32_t* d_pssm, int32_t pssm_stride,
                       mss_scoring_t sc, int32_t pad, void* ws, size_t ws_bytes, cudaStream_t st,
                       int32_t* d_score, int64_t* d_ref_pos, uint32_t* d_cigar, int32_t cigar_stride, int32_t* d_n_cigar)
 {
@@ -249,6 +262,7 @@ cudaError_t launch_nw(const mss_genome* g, const uint32_t* d_reads, const uint32
     p.reads = d_reads; p.reads_nmask = d_reads_nmask; p.stride_words = stride_words; p.lens = d_lens;
     p.n_reads = n_reads; p.max_len = max_len; p.hits = d_hits;
     p.match = sc.match; p.mismatch = sc.mismatch; p.gap = sc.gap; p.pad = pad;
+    p.pssm = d_pssm; p.pssm_stride = pssm_stride;
     p.score = d_score; p.ref_pos = d_ref_pos; p.cigar = d_cigar; p.cigar_stride = cigar_stride; p.n_cigar = d_n_cigar;
     int32_t* base = (int32_t*)ws;
     p.bnd = base; p.bnd_stride = (int64_t)ge.bnd_stride;

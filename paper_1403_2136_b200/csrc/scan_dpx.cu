@@ -37,7 +37,17 @@ __device__ __forceinline__ uint32_t pack2(int32_t lo, int32_t hi)
     return ((uint32_t)lo & 0xFFFFu) | ((uint32_t)hi << 16);
 }
 
-template <int K, int T>
+// select per lane: mask lane 0xFFFF -> a, 0x0000 -> b (one LOP3)
+__device__ __forceinline__ uint32_t lane_select(uint32_t mask, uint32_t a, uint32_t b)
+{
+    return (mask & a) | (~mask & b);
+}
+
+// PSSM = false: the two global scores are baked into the planes (the paper's "trivial match or mismatch cost").
+// PSSM = true : the planes hold equality masks and every step selects the query position's own (pmatch, pmismatch)
+//               (base-quality position-specific scoring): one extra LOP3 per 2 cells.
+// p.istep = 2 (MaxSSmap_fast) only changes the tables built in a1: step j reads read position 2j.
+template <int K, int T, bool PSSM>
 __global__ void __launch_bounds__(T)
 scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2_t* __restrict__ out_partial)
 {
@@ -45,7 +55,8 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t* planes = smem;                                   // 5 * ROWW
     uint32_t* roff = planes + 5 * ROWW;                        // NQ_MAX * MP
-    uint32_t* wres = roff + NQ_MAX * MP;                       // NQ_MAX * NW
+    uint2* pq = reinterpret_cast<uint2*>(roff + NQ_MAX * MP);  // PSSM only: NQ_MAX * MP packed (pmatch x2, pmismatch x2)
+    uint32_t* wres = roff + NQ_MAX * MP + (PSSM ? 2 * NQ_MAX * MP : 0);   // NQ_MAX * NW
     int32_t* qlen = (int32_t*)(wres + NQ_MAX * C::NW);         // NQ_MAX
     unsigned long long* cur = (unsigned long long*)(qlen + NQ_MAX);   // NQ_MAX (per read; 8-byte aligned by layout)
     mss_hit_t* tbest = (mss_hit_t*)(cur + NQ_MAX);             // NQ_MAX
@@ -69,11 +80,20 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
         bool ok = (m >= 1 && m <= p.max_len);
         const uint32_t* rw = p.reads + (int64_t)r * p.stride_words;
         const uint32_t* rn = p.reads_nmask ? p.reads_nmask + (int64_t)r * ((p.stride_words + 1) / 2) : nullptr;
-        for (int32_t i = lane; i < MP; i += 32) {
-            uint32_t b = (ok && i < m) ? read_base(rw, rn, m, i, strand) : 4u;
-            roff[q * MP + i] = (b * (uint32_t)ROWW + (uint32_t)i) * 4u;      // byte offset into the planes
+        const uint32_t* prow = PSSM ? p.pssm + (int64_t)r * p.pssm_stride : nullptr;
+        for (int32_t j = lane; j < MP; j += 32) {
+            const int32_t i = j * p.istep;                      // read position scored at step j
+            const bool live = ok && i < m;
+            uint32_t b = live ? read_base(rw, rn, m, i, strand) : 4u;
+            uint32_t col = live ? (uint32_t)i : (uint32_t)j;    // dead steps: any column of the all-mismatch plane
+            roff[q * MP + j] = (b * (uint32_t)ROWW + col) * 4u; // byte offset into the planes
+            if (PSSM) {
+                uint32_t w = live ? pssm_at(prow, m, i, strand) : 0u;      // dead steps add 0
+                uint32_t mt = w & 0xFFFFu, mm = w >> 16;
+                pq[q * MP + j] = make_uint2(mt | (mt << 16), mm | (mm << 16));
+            }
         }
-        if (lane == 0) qlen[q] = ok ? m : 0;
+        if (lane == 0) qlen[q] = ok ? (m + p.istep - 1) / p.istep : 0;     // number of steps
     }
     if (tid < NQ_MAX) {
         cur[tid] = 0ull;
@@ -100,10 +120,11 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
                 int64_t plo = g0 + x, phi = plo + C::HALF;
                 uint32_t lo = plo < trunc ? base_at(p.gpacked, p.gnmask, plo) : 4u;
                 uint32_t hi = phi < trunc ? base_at(p.gpacked, p.gnmask, phi) : 4u;
+                const int32_t eqv = PSSM ? -1 : p.match, nev = PSSM ? 0 : p.mismatch;
 #pragma unroll
                 for (uint32_t c = 0; c < 4; c++)
-                    planes[c * ROWW + x] = pack2(lo == c ? p.match : p.mismatch, hi == c ? p.match : p.mismatch);
-                planes[4 * ROWW + x] = pack2(p.mismatch, p.mismatch);
+                    planes[c * ROWW + x] = pack2(lo == c ? eqv : nev, hi == c ? eqv : nev);
+                planes[4 * ROWW + x] = pack2(nev, nev);
             }
             __syncthreads();
 
@@ -119,18 +140,39 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
                 for (int32_t i0 = 0; i0 < m; i0 += 4) {
                     const uint4 o = *reinterpret_cast<const uint4*>(ro + i0);
                     uint32_t Ha[K];
+                    if (!PSSM) {
 #pragma unroll
-                    for (int k = 0; k < K; k++) Ha[k] = __viaddmax_s16x2(H[k], *reinterpret_cast<const uint32_t*>(my + o.x + k * T * 4), zero);
+                        for (int k = 0; k < K; k++) Ha[k] = __viaddmax_s16x2(H[k], *reinterpret_cast<const uint32_t*>(my + o.x + k * T * 4), zero);
 #pragma unroll
-                    for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.y + k * T * 4), zero);
+                        for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.y + k * T * 4), zero);
 #pragma unroll
-                    for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                        for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
 #pragma unroll
-                    for (int k = 0; k < K; k++) Ha[k] = __viaddmax_s16x2(H[k], *reinterpret_cast<const uint32_t*>(my + o.z + k * T * 4), zero);
+                        for (int k = 0; k < K; k++) Ha[k] = __viaddmax_s16x2(H[k], *reinterpret_cast<const uint32_t*>(my + o.z + k * T * 4), zero);
 #pragma unroll
-                    for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.w + k * T * 4), zero);
+                        for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.w + k * T * 4), zero);
 #pragma unroll
-                    for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                        for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                    } else {
+                        const uint4 s01 = *reinterpret_cast<const uint4*>(pq + q * MP + i0);        // (mt0, mm0, mt1, mm1)
+                        const uint4 s23 = *reinterpret_cast<const uint4*>(pq + q * MP + i0 + 2);
+#pragma unroll
+                        for (int k = 0; k < K; k++)
+                            Ha[k] = __viaddmax_s16x2(H[k], lane_select(*reinterpret_cast<const uint32_t*>(my + o.x + k * T * 4), s01.x, s01.y), zero);
+#pragma unroll
+                        for (int k = 0; k < K; k++)
+                            H[k] = __viaddmax_s16x2(Ha[k], lane_select(*reinterpret_cast<const uint32_t*>(my + o.y + k * T * 4), s01.z, s01.w), zero);
+#pragma unroll
+                        for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+#pragma unroll
+                        for (int k = 0; k < K; k++)
+                            Ha[k] = __viaddmax_s16x2(H[k], lane_select(*reinterpret_cast<const uint32_t*>(my + o.z + k * T * 4), s23.x, s23.y), zero);
+#pragma unroll
+                        for (int k = 0; k < K; k++)
+                            H[k] = __viaddmax_s16x2(Ha[k], lane_select(*reinterpret_cast<const uint32_t*>(my + o.w + k * T * 4), s23.z, s23.w), zero);
+#pragma unroll
+                        for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                    }
                 }
                 // a4: warp max and its lowest window start
                 if (nvalid < C::D) {                            // ragged last tile of a fragment: drop foreign window starts
@@ -233,20 +275,34 @@ DpxUnitGeom unit_geom(const mss_genome* g, int32_t n_reads, int32_t strands)
 struct Variant { int id, K, T; };
 const Variant kVariants[] = { {2, 8, 256}, {3, 8, 128}, {4, 8, 64}, {5, 4, 256}, {6, 16, 128} };
 
-template <int K, int T>
-cudaError_t launch_variant(const mss_genome* g, const ScanParams& p, const DpxUnitGeom& ug, mss_top2_t* partial,
-                           cudaStream_t st, mss_launch_info_t* info, int id)
+// shared-memory geometry: MP = steps per query rounded to 4 (table rows), ROWW = plane columns (tile half + read length)
+struct SmemGeom { int32_t MP, ROWW; size_t bytes; };
+SmemGeom smem_geom(int half, int nw, int32_t max_len, int32_t istep, bool pssm)
+{
+    SmemGeom s;
+    int32_t steps = (max_len + istep - 1) / istep;
+    s.MP = (steps + 3) & ~3;
+    int32_t MPL = (max_len + 3) & ~3;
+    if (MPL < s.MP) MPL = s.MP;
+    s.ROWW = (half + MPL + 3) & ~3;
+    s.bytes = (size_t)(5 * s.ROWW + NQ_MAX * s.MP * (pssm ? 3 : 1) + NQ_MAX * nw) * 4 + NQ_MAX * 4 + NQ_MAX * 8
+            + 2 * NQ_MAX * sizeof(mss_hit_t) + NQ_MAX * 4;
+    return s;
+}
+
+template <int K, int T, bool PSSM>
+cudaError_t launch_variant2(const mss_genome* g, const ScanParams& p, const DpxUnitGeom& ug, mss_top2_t* partial,
+                            cudaStream_t st, mss_launch_info_t* info, int id)
 {
     using C = Cfg<K, T>;
-    int32_t MP = (p.max_len + 3) & ~3;
-    int32_t ROWW = (C::HALF + MP + 3) & ~3;
-    size_t smem = (size_t)(5 * ROWW + NQ_MAX * MP + NQ_MAX * C::NW) * 4 + NQ_MAX * 4 + NQ_MAX * 8 + 2 * NQ_MAX * sizeof(mss_hit_t)
-                + NQ_MAX * 4;
+    SmemGeom sg = smem_geom(C::HALF, C::NW, p.max_len, p.istep, PSSM);
+    int32_t MP = sg.MP, ROWW = sg.ROWW;
+    size_t smem = sg.bytes;
     if (smem > (size_t)g->max_smem_optin) return cudaErrorInvalidConfiguration;
-    cudaError_t e = cudaFuncSetAttribute(scan_dpx_kernel<K, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(scan_dpx_kernel<K, T, PSSM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int64_t blocks = (int64_t)ug.n_groups * ug.n_splits;
-    scan_dpx_kernel<K, T><<<(unsigned)blocks, T, smem, st>>>(p, ug, MP, ROWW, partial);
+    scan_dpx_kernel<K, T, PSSM><<<(unsigned)blocks, T, smem, st>>>(p, ug, MP, ROWW, partial);
     if (info) {
         info->variant = id; info->grid = (int32_t)blocks; info->block = T; info->smem_bytes = (int32_t)smem;
         info->reads_per_block = ug.reads_per_group; info->tile_diagonals = C::D; info->launches = 2;
@@ -254,13 +310,26 @@ cudaError_t launch_variant(const mss_genome* g, const ScanParams& p, const DpxUn
     return cudaGetLastError();
 }
 
-int pick_variant(const mss_genome* g, int requested)
+template <int K, int T>
+cudaError_t launch_variant(const mss_genome* g, const ScanParams& p, const DpxUnitGeom& ug, mss_top2_t* partial,
+                           cudaStream_t st, mss_launch_info_t* info, int id)
 {
-    for (const Variant& v : kVariants) if (v.id == requested) return requested;
-    // automatic: the tile size with the least padding waste, larger tiles preferred on ties
-    int best = 2; double best_waste = 1e30;
+    return p.pssm ? launch_variant2<K, T, true>(g, p, ug, partial, st, info, id)
+                  : launch_variant2<K, T, false>(g, p, ug, partial, st, info, id);
+}
+
+bool variant_fits(const mss_genome* g, const ScanParams& p, const Variant& v)
+{
+    return smem_geom(v.K * v.T, v.T / 32, p.max_len, p.istep, p.pssm != nullptr).bytes <= (size_t)g->max_smem_optin;
+}
+
+int pick_variant(const mss_genome* g, const ScanParams& p, int requested)
+{
+    for (const Variant& v : kVariants) if (v.id == requested && variant_fits(g, p, v)) return requested;
+    // automatic: among the tiles whose shared memory fits, the one with the least padding waste (larger tiles on ties)
+    int best = 4; double best_waste = 1e30;
     for (const Variant& v : kVariants) {
-        if (v.id > 4) continue;                                  // 5, 6 are tuning variants, never automatic
+        if (v.id > 4 || !variant_fits(g, p, v)) continue;        // 5, 6 are tuning variants, never automatic
         int D = 2 * v.K * v.T;
         double waste = (double)((g->frag_len + D - 1) / D) * D / g->frag_len;
         if (waste < best_waste - 1e-9) { best_waste = waste; best = v.id; }
@@ -274,9 +343,7 @@ bool scan_dpx_supported(const mss_genome* g, const ScanParams& p)
 {
     if (g->frag_len < 256) return false;                        // tiles would be mostly padding: generic kernel
     if ((int64_t)p.max_len * p.match > 32767 || p.mismatch < -32768) return false;
-    int32_t MP = (p.max_len + 3) & ~3;
-    size_t smem_min = (size_t)(5 * (512 + MP + 4) + NQ_MAX * MP + NQ_MAX * 8) * 4 + 4096;
-    return smem_min <= (size_t)g->max_smem_optin;
+    return smem_geom(512, 2, p.max_len, p.istep, p.pssm != nullptr).bytes <= (size_t)g->max_smem_optin;   // smallest tile (K8,T64)
 }
 
 size_t scan_dpx_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, int32_t strands)
@@ -292,7 +359,7 @@ cudaError_t launch_scan_dpx(const mss_genome* g, const ScanParams& p, void* ws, 
     (void)ws_bytes;
     DpxUnitGeom ug = unit_geom(g, p.n_reads, p.strands);
     mss_top2_t* partial = (mss_top2_t*)ws;
-    int id = pick_variant(g, variant);
+    int id = pick_variant(g, p, variant);
     cudaError_t e;
     switch (id) {
         case 3: e = launch_variant<8, 128>(g, p, ug, partial, st, info, id); break;

@@ -8,7 +8,9 @@
 __global__ void __launch_bounds__(GEN_THREADS)
 scan_generic_kernel(ScanParams p, int32_t read0, int32_t chunk_reads, uint64_t* __restrict__ fragkey)
 {
-    extern __shared__ uint8_t q[];                      // strand-oriented read, one byte per base
+    extern __shared__ __align__(8) uint8_t gsm[];
+    int32_t* qs = reinterpret_cast<int32_t*>(gsm);      // PSSM only: (pmatch, pmismatch) of the strand-oriented read
+    uint8_t* q = gsm + (p.pssm ? (size_t)p.max_len * 8 : 0);   // strand-oriented read, one byte per base
     __shared__ uint64_t wmax[GEN_THREADS / 32];
     int64_t bid = blockIdx.x;
     int32_t rl = (int32_t)(bid % chunk_reads);
@@ -20,20 +22,29 @@ scan_generic_kernel(ScanParams p, int32_t read0, int32_t chunk_reads, uint64_t* 
     if (m >= 1 && m <= p.max_len) {
         const uint32_t* rw = p.reads + (int64_t)r * p.stride_words;
         const uint32_t* rn = p.reads_nmask ? p.reads_nmask + (int64_t)r * ((p.stride_words + 1) / 2) : nullptr;
+        const uint32_t* prow = p.pssm ? p.pssm + (int64_t)r * p.pssm_stride : nullptr;
         int32_t veff = (p.V < 0 || p.V > m - 1) ? m - 1 : p.V;
         int64_t fstart = (int64_t)f * p.F, end = fstart + p.F + veff;
         for (int32_t s = 0; s < 2; s++) {
             if (!(p.strands & (1 << s))) continue;
             __syncthreads();
-            for (int32_t i = threadIdx.x; i < m; i += GEN_THREADS) q[i] = (uint8_t)read_base(rw, rn, m, i, s);
+            for (int32_t i = threadIdx.x; i < m; i += GEN_THREADS) {
+                q[i] = (uint8_t)read_base(rw, rn, m, i, s);
+                if (prow) {
+                    uint32_t w = pssm_at(prow, m, i, s);
+                    qs[2 * i] = (int32_t)(int16_t)(w & 0xFFFFu);
+                    qs[2 * i + 1] = (int32_t)(int16_t)(w >> 16);
+                }
+            }
             __syncthreads();
             for (int32_t d = threadIdx.x; d < p.F; d += GEN_THREADS) {
                 int64_t g = fstart + d;
                 int32_t n = (end - g < m) ? (int32_t)(end - g) : m;
                 int32_t H = 0, b = 0;
-                for (int32_t i = 0; i < n; i++) {
+                for (int32_t i = 0; i < n; i += p.istep) {
                     uint32_t gb = base_at(p.gpacked, p.gnmask, g + i);
-                    int32_t sc = (gb < 4u && gb == q[i]) ? p.match : p.mismatch;
+                    bool eq = gb < 4u && gb == q[i];
+                    int32_t sc = prow ? (eq ? qs[2 * i] : qs[2 * i + 1]) : (eq ? p.match : p.mismatch);
                     H = max(H + sc, 0);
                     b = max(b, H);
                 }
@@ -102,10 +113,18 @@ cudaError_t launch_scan_generic(const mss_genome* g, const ScanParams& p, void* 
     int32_t chunk = generic_chunk(g, p.n_reads);
     uint64_t* fragkey = (uint64_t*)ws;
     int launches = 0;
+    {
+        size_t smem = (size_t)p.max_len + 16 + (p.pssm ? (size_t)p.max_len * 8 : 0);
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(scan_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+    }
     for (int32_t r0 = 0; r0 < p.n_reads; r0 += chunk) {
         int32_t c = p.n_reads - r0 < chunk ? p.n_reads - r0 : chunk;
         int64_t blocks = (int64_t)c * g->n_frag;
-        scan_generic_kernel<<<(unsigned)blocks, GEN_THREADS, (size_t)p.max_len + 16, st>>>(p, r0, c, fragkey);
+        size_t smem = (size_t)p.max_len + 16 + (p.pssm ? (size_t)p.max_len * 8 : 0);
+        scan_generic_kernel<<<(unsigned)blocks, GEN_THREADS, smem, st>>>(p, r0, c, fragkey);
         top2_over_fragments_kernel<<<(c + 127) / 128, 128, 0, st>>>(p, r0, c, fragkey, d_out);
         launches += 2;
         if (info) { info->grid = (int32_t)blocks; }
