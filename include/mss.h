@@ -252,9 +252,11 @@ int mss_probe_dpx_peak(int32_t iters, void *stream, double *h_instr_per_s, float
  * steps on 1024 threads per SM.  0 VIADDMNMX.S16x2.RELU, 1 VIMNMX3.S16x2, 2 their 2:1 mix, 3 PRMT, 4 LOP3, 5 IMAD,
  * 6 HFMA2.RELU, 7 DPX+IMAD, 8 DPX+PRMT, 9 DPX+HFMA2.RELU (both counted), 10 LDS.32, 11 the scan's inner mix
  * (LDS.32 + VIADDMNMX per 2 cells + VIMNMX3 per 4 cells), 12 PRMT + HFMA2.RELU + VIMNMX3 mix, 13 PRMT + VIADDMNMX +
- * VIMNMX3 mix.  Synchronises the stream before returning.
+ * VIMNMX3 mix, 14 F2FP.F16.E4M3.UNPACK_B (fp8 pair -> f16x2), 15 DPX+F2FP, 16 HFMA2+F2FP (both counted), 17 byte-score mix
+ * (LDS.32 per 4 cells + 2 F2FP + 2 HFMA2.RELU + VIMNMX3) [cells], 18 the same with PRMT as the widening [cells],
+ * 19 hybrid of rows 11 and 17 on alternating chains [cells].  Synchronises the stream before returning.
  */
-enum { MSS_PROBE_COUNT = 14 };
+enum { MSS_PROBE_COUNT = 20 };
 int mss_probe_pipe(int32_t which, int32_t iters, void *stream, double *h_per_clk_sm);
 
 #ifdef __cplusplus

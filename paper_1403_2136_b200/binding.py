@@ -366,7 +366,11 @@ PROBE_NAMES = ["VIADDMNMX.S16x2.RELU", "VIMNMX3.S16x2", "DPX mix 2:1 (relu : max
                "DPX + IMAD 1:1 (both counted)", "DPX + PRMT 1:1 (both counted)", "DPX + HFMA2.RELU 1:1 (both counted)",
                "LDS.32 (conflict-free)", "scan mix: LDS.32 + VIADDMNMX /2 cells + VIMNMX3 /4 cells  [cells]",
                "alt mix: PRMT + HFMA2.RELU /2 cells + VIMNMX3 /4 cells  [cells]",
-               "alt mix: PRMT + VIADDMNMX /2 cells + VIMNMX3 /4 cells  [cells]"]
+               "alt mix: PRMT + VIADDMNMX /2 cells + VIMNMX3 /4 cells  [cells]",
+               "F2FP.F16.E4M3.UNPACK_B (fp8x2 -> f16x2)", "DPX + F2FP 1:1 (both counted)", "HFMA2.RELU + F2FP 1:1 (both counted)",
+               "byte mix: LDS.32 /4 cells + 2 F2FP + 2 HFMA2.RELU + VIMNMX3  [cells]",
+               "byte mix: LDS.32 /4 cells + 2 PRMT + 2 HFMA2.RELU + VIMNMX3  [cells]",
+               "hybrid: chains alternate scan mix (row 11) and byte mix (row 17)  [cells]"]
 
 
 def mss_probe_pipe(which: int, iters: int = 2000, stream=None) -> float:

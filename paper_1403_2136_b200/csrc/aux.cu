@@ -106,6 +106,16 @@ __device__ __forceinline__ uint32_t p_imad(uint32_t a, uint32_t b, uint32_t c) {
 __device__ __forceinline__ uint32_t p_hfma2r(uint32_t a, uint32_t b, uint32_t c) { uint32_t d; asm volatile("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c)); return d; }
 __device__ __forceinline__ uint32_t p_lop3(uint32_t a, uint32_t b, uint32_t c) { uint32_t d; asm volatile("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(d) : "r"(a), "r"(b), "r"(c)); return d; }
 
+// fp8 e4m3 pair -> f16x2 (F2FP.F16.E4M3.UNPACK_B); HI selects the upper 16 bits of the source (operand .H1, no shift)
+template <bool HI>
+__device__ __forceinline__ uint32_t p_f2fp(uint32_t w)
+{
+    uint32_t d;
+    if (HI) asm volatile("{ .reg .b16 lo, hi; mov.b32 {lo, hi}, %1; cvt.rn.f16x2.e4m3x2 %0, hi; }" : "=r"(d) : "r"(w));
+    else    asm volatile("{ .reg .b16 lo, hi; mov.b32 {lo, hi}, %1; cvt.rn.f16x2.e4m3x2 %0, lo; }" : "=r"(d) : "r"(w));
+    return d;
+}
+
 template <int WHICH>
 __global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long long* cyc, uint32_t a, uint32_t b, uint32_t c, int iters)
 {
@@ -149,6 +159,33 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long lo
                     if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
                     h[j] = hn;
                 }
+                if (WHICH == 14) h[j] = p_f2fp<false>(h[j]) ^ 0u;
+                if (WHICH == 15) { h[j] = __viaddmax_s16x2_relu(h[j], b, c); m[j] = p_f2fp<true>(m[j]); }
+                if (WHICH == 16) { h[j] = p_hfma2r(h[j], b, c); m[j] = p_f2fp<true>(m[j]); }
+                if (WHICH == 17 || WHICH == 18) {
+                    // byte-score mixes: one LDS.32 carries 4 cells (fp8 / byte scores); per 4 cells 2 widenings
+                    // (17: F2FP e4m3x2->f16x2, 18: PRMT) + 2 HFMA2.RELU (Kadane in exact fp16) + 1 VIMNMX3.S16x2
+                    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(myp + ((u * 8 + j) & 63) * 32 + (it & 1) * 2048)));
+                    uint32_t s0 = WHICH == 17 ? p_f2fp<false>(v) : p_prmt(v, c, 0x1404u);
+                    uint32_t s1 = WHICH == 17 ? p_f2fp<true>(v) : p_prmt(v, c, 0x3424u);
+                    uint32_t h1 = p_hfma2r(h[j], a, s0);
+                    uint32_t h2 = p_hfma2r(h1, a, s1);
+                    m[j] = __vimax3_s16x2(m[j], h1, h2);
+                    h[j] = h2;
+                }
+                if (WHICH == 19) {   // hybrid: even chains as row 11 (LDS.32 + DPX per 2 cells), odd chains as row 17 at half rate
+                    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(myp + ((u * 8 + j) & 63) * 32 + (it & 1) * 2048)));
+                    if (j & 1) {
+                        uint32_t h1 = p_hfma2r(h[j], a, p_f2fp<false>(v));
+                        uint32_t h2 = p_hfma2r(h1, a, p_f2fp<true>(v));
+                        m[j] = __vimax3_s16x2(m[j], h1, h2);
+                        h[j] = h2;
+                    } else {
+                        uint32_t hn = __viaddmax_s16x2_relu(h[j], v, c);
+                        if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
+                        h[j] = hn;
+                    }
+                }
                 if (WHICH == 13) {   // alternative mix, all on the ALU pipe: PRMT + VIADDMNMX per 2 cells, VIMNMX3 per 4 cells
                     uint32_t sc = p_prmt(m[j], b, h[(j + 1) & 7]);
                     uint32_t hn = __viaddmax_s16x2_relu(h[j], sc, c);
@@ -166,7 +203,7 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long lo
     if (threadIdx.x == 0) cyc[blockIdx.x] = t1 - t0;
 }
 
-const double kProbeCount[14] = { 1, 1, 1.5, 1, 1, 1, 1, 2, 2, 2, 1, 2, 2, 2 };   // counted units per chain step (mix rows 11-13: cells)
+const double kProbeCount[20] = { 1, 1, 1.5, 1, 1, 1, 1, 2, 2, 2, 1, 2, 2, 2, 1, 2, 2, 4, 4, 3 };   // counted units per chain step (mix rows 11-13: cells)
 
 template <int WHICH>
 cudaError_t launch_pipe_probe(uint32_t* out, long long* cyc, int blocks, int iters, cudaStream_t st)
@@ -178,7 +215,7 @@ cudaError_t launch_pipe_probe(uint32_t* out, long long* cyc, int blocks, int ite
 
 cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_count, double* per_clk_sm)
 {
-    if (which < 0 || which > 13) return cudaErrorInvalidValue;
+    if (which < 0 || which > 19) return cudaErrorInvalidValue;
     uint32_t* out = nullptr; long long* cyc = nullptr;
     int blocks = sm_count;
     cudaError_t e = cudaMalloc(&out, (size_t)blocks * 1024 * 4);                 // probe only: not on the mapping path
@@ -199,7 +236,13 @@ cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_cou
             case 10: e = launch_pipe_probe<10>(out, cyc, blocks, iters, st); break;
             case 11: e = launch_pipe_probe<11>(out, cyc, blocks, iters, st); break;
             case 12: e = launch_pipe_probe<12>(out, cyc, blocks, iters, st); break;
-            default: e = launch_pipe_probe<13>(out, cyc, blocks, iters, st); break;
+            case 13: e = launch_pipe_probe<13>(out, cyc, blocks, iters, st); break;
+            case 14: e = launch_pipe_probe<14>(out, cyc, blocks, iters, st); break;
+            case 15: e = launch_pipe_probe<15>(out, cyc, blocks, iters, st); break;
+            case 16: e = launch_pipe_probe<16>(out, cyc, blocks, iters, st); break;
+            case 17: e = launch_pipe_probe<17>(out, cyc, blocks, iters, st); break;
+            case 18: e = launch_pipe_probe<18>(out, cyc, blocks, iters, st); break;
+            default: e = launch_pipe_probe<19>(out, cyc, blocks, iters, st); break;
         }
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
