@@ -254,9 +254,10 @@ int mss_probe_dpx_peak(int32_t iters, void *stream, double *h_instr_per_s, float
  * (LDS.32 + VIADDMNMX per 2 cells + VIMNMX3 per 4 cells), 12 PRMT + HFMA2.RELU + VIMNMX3 mix, 13 PRMT + VIADDMNMX +
  * VIMNMX3 mix, 14 F2FP.F16.E4M3.UNPACK_B (fp8 pair -> f16x2), 15 DPX+F2FP, 16 HFMA2+F2FP (both counted), 17 byte-score mix
  * (LDS.32 per 4 cells + 2 F2FP + 2 HFMA2.RELU + VIMNMX3) [cells], 18 the same with PRMT as the widening [cells],
- * 19 hybrid of rows 11 and 17 on alternating chains [cells].  Synchronises the stream before returning.
+ * 19 hybrid of rows 11 and 17 on alternating chains [cells], 20 LDS.64, 21 LDS.128 (thread-loads; x8 / x16 bytes).
+ * Synchronises the stream before returning.
  */
-enum { MSS_PROBE_COUNT = 20 };
+enum { MSS_PROBE_COUNT = 22 };
 int mss_probe_pipe(int32_t which, int32_t iters, void *stream, double *h_per_clk_sm);
 
 #ifdef __cplusplus

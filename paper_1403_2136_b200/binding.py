@@ -370,7 +370,8 @@ PROBE_NAMES = ["VIADDMNMX.S16x2.RELU", "VIMNMX3.S16x2", "DPX mix 2:1 (relu : max
                "F2FP.F16.E4M3.UNPACK_B (fp8x2 -> f16x2)", "DPX + F2FP 1:1 (both counted)", "HFMA2.RELU + F2FP 1:1 (both counted)",
                "byte mix: LDS.32 /4 cells + 2 F2FP + 2 HFMA2.RELU + VIMNMX3  [cells]",
                "byte mix: LDS.32 /4 cells + 2 PRMT + 2 HFMA2.RELU + VIMNMX3  [cells]",
-               "hybrid: chains alternate scan mix (row 11) and byte mix (row 17)  [cells]"]
+               "hybrid: chains alternate scan mix (row 11) and byte mix (row 17)  [cells]",
+               "LDS.64 (conflict-free; x8 bytes)", "LDS.128 (conflict-free; x16 bytes)"]
 
 
 def mss_probe_pipe(which: int, iters: int = 2000, stream=None) -> float:

@@ -186,6 +186,14 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long lo
                         h[j] = hn;
                     }
                 }
+                if (WHICH == 20) {   // LDS.64 (conflict-free): bytes per clock, not instructions, are what it shows
+                    uint32_t v0, v1; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v0), "=r"(v1) : "r"((uint32_t)__cvta_generic_to_shared(sm + 2 * threadIdx.x + ((u * 8 + j) & 1) * 2048 + ((h[j] >> 7) & 1) * 4096)));
+                    h[j] ^= v0; m[j] ^= v1;
+                }
+                if (WHICH == 21) {   // LDS.128 (conflict-free)
+                    uint32_t v0, v1, v2, v3; asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3) : "r"((uint32_t)__cvta_generic_to_shared(sm + 4 * threadIdx.x + ((h[j] >> 7) & 1) * 4096)));
+                    h[j] ^= v0 ^ v2; m[j] ^= v1 ^ v3;
+                }
                 if (WHICH == 13) {   // alternative mix, all on the ALU pipe: PRMT + VIADDMNMX per 2 cells, VIMNMX3 per 4 cells
                     uint32_t sc = p_prmt(m[j], b, h[(j + 1) & 7]);
                     uint32_t hn = __viaddmax_s16x2_relu(h[j], sc, c);
@@ -203,7 +211,7 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long lo
     if (threadIdx.x == 0) cyc[blockIdx.x] = t1 - t0;
 }
 
-const double kProbeCount[20] = { 1, 1, 1.5, 1, 1, 1, 1, 2, 2, 2, 1, 2, 2, 2, 1, 2, 2, 4, 4, 3 };   // counted units per chain step (mix rows 11-13: cells)
+const double kProbeCount[22] = { 1, 1, 1.5, 1, 1, 1, 1, 2, 2, 2, 1, 2, 2, 2, 1, 2, 2, 4, 4, 3, 1, 1 };   // counted units per chain step (mix rows 11-13: cells)
 
 template <int WHICH>
 cudaError_t launch_pipe_probe(uint32_t* out, long long* cyc, int blocks, int iters, cudaStream_t st)
@@ -215,7 +223,7 @@ cudaError_t launch_pipe_probe(uint32_t* out, long long* cyc, int blocks, int ite
 
 cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_count, double* per_clk_sm)
 {
-    if (which < 0 || which > 19) return cudaErrorInvalidValue;
+    if (which < 0 || which > 21) return cudaErrorInvalidValue;
     uint32_t* out = nullptr; long long* cyc = nullptr;
     int blocks = sm_count;
     cudaError_t e = cudaMalloc(&out, (size_t)blocks * 1024 * 4);                 // probe only: not on the mapping path
@@ -242,7 +250,9 @@ cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_cou
             case 16: e = launch_pipe_probe<16>(out, cyc, blocks, iters, st); break;
             case 17: e = launch_pipe_probe<17>(out, cyc, blocks, iters, st); break;
             case 18: e = launch_pipe_probe<18>(out, cyc, blocks, iters, st); break;
-            default: e = launch_pipe_probe<19>(out, cyc, blocks, iters, st); break;
+            case 19: e = launch_pipe_probe<19>(out, cyc, blocks, iters, st); break;
+            case 20: e = launch_pipe_probe<20>(out, cyc, blocks, iters, st); break;
+            default: e = launch_pipe_probe<21>(out, cyc, blocks, iters, st); break;
         }
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
