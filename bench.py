@@ -136,6 +136,10 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); the metric is quoted on 2")
     ap.add_argument("--reads", type=int, default=None, help="reads per step per GPU (default: the config's own count)")
     ap.add_argument("--variant", type=int, default=0, help="scan kernel variant (0 = automatic)")
+    ap.add_argument("--read-len", type=int, default=None,
+                    help="diagnostic: keep only the config's read groups of this length (config 3's sweep, one length at a time)")
+    ap.add_argument("--mode", default="plain", choices=["plain", "fast", "pssm"],
+                    help="diagnostic: time the next-row scans (MaxSSmap_fast / base-quality PSSM) instead of the plain scan")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-nw", action="store_true", help="time the MaxSS stage only (diagnostic; not a bench value)")
     ap.add_argument("--ref-reads-per-core", type=int, default=2)
@@ -163,16 +167,19 @@ def main():
 
     # ---- inputs: genome replicated, reads sharded by rank (independent units, no data-path collective) ------------
     genome, _ = cfg.genome()
-    m = cfg.max_len
-    n_reads = args.reads or cfg.n_reads
-    if args.reads is None:
+    groups = [g for g in cfg.groups if args.read_len in (None, g[1])]
+    if not groups:
+        raise SystemExit(f"config {cfg.c} has no read group of length {args.read_len}")
+    m = max(g[1] for g in groups)
+    n_reads = args.reads or sum(g[0] for g in groups)
+    if args.reads is None and args.read_len is None:
         r = cfg.reads(genome) if world == 1 else None
     else:
         r = None
     if r is None:   # ranks draw their own batch (weak scaling): same recipe, seed offset by rank
         outs = []
-        per = max(1, n_reads // len(cfg.groups))
-        for gi, (_, mm, rate) in enumerate(cfg.groups):
+        per = max(1, n_reads // len(groups))
+        for gi, (_, mm, rate) in enumerate(groups):
             o = gen.make_reads(genome, per, mm, cfg.reads_seed + 100 * gi + 7919 * rank, sub_rate=rate,
                                indel_prob=cfg.indel_prob, both_strands=cfg.both_strands, avoid_n=cfg.avoid_n)
             if mm < m:
@@ -199,16 +206,30 @@ def main():
     mss.mss_set_scan_variant(args.variant)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)          # > 126 MB L2
     stream = torch.cuda.current_stream()
-    cells_step = float(np.sum(lens.astype(np.float64))) * G.n_frag * cfg.frag_len * (2 if cfg.strands == 3 else 1)
+    scored = lens.astype(np.float64) if args.mode != "fast" else np.ceil(lens.astype(np.float64) / 2)   # fast: every other base
+    cells_step = float(np.sum(scored)) * G.n_frag * cfg.frag_len * (2 if cfg.strands == 3 else 1)
+    d_qual, pssm_scale = None, 16
+    if args.mode == "pssm":
+        d_qual = torch.from_numpy(gen.make_quals(n_reads, m, cfg.reads_seed + 5)).to(dev)
 
     def step():
         """resident inputs -> top-2 records -> NW score/pos/CIGAR, all on the device; returns (scan_ms event pair)."""
         e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         e0.record(stream)
-        top2 = mss.mss_map_reads(G, d_reads, d_mask, d_lens, m, sc, cfg.strands)
+        if args.mode == "fast":
+            top2 = mss.mss_map_reads_fast(G, d_reads, d_mask, d_lens, m, sc, cfg.strands)
+        elif args.mode == "pssm":
+            d_pssm = mss.mss_pssm_build(d_qual, d_lens, sc, pssm_scale)
+            bound = mss.pssm_bound(sc, pssm_scale)
+            top2 = mss.mss_map_reads_pssm(G, d_reads, d_mask, d_lens, m, d_pssm, bound, cfg.strands)
+        else:
+            top2 = mss.mss_map_reads(G, d_reads, d_mask, d_lens, m, sc, cfg.strands)
         e1.record(stream)
         if not args.no_nw:
-            mss.mss_nw_align(G, d_reads, d_mask, d_lens, m, top2, sc, 30, args.cigar_stride)
+            if args.mode == "pssm":
+                mss.mss_nw_align_pssm(G, d_reads, d_mask, d_lens, m, top2, d_pssm, bound, 30, args.cigar_stride)
+            else:
+                mss.mss_nw_align(G, d_reads, d_mask, d_lens, m, top2, sc, 30, args.cigar_stride)
         e2.record(stream)
         return e0, e1, e2, top2
 
@@ -247,22 +268,27 @@ def main():
     ms_per_step = total_ms / args.steps
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region ----------------------------------------
-    out = mss.mss_map_align_host(G, h_reads, h_mask, h_lens, m, sc, cfg.strands, 30, args.cigar_stride)   # warm-up
-    e2e_times = []
-    for _ in range(max(1, min(args.steps, 2))):
-        flush.fill_(1)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        out = mss.mss_map_align_host(G, h_reads, h_mask, h_lens, m, sc, cfg.strands, 30, args.cigar_stride, out=out)
-        e2e_times.append(time.perf_counter() - t0)
-    e2e_s = sum(e2e_times) / len(e2e_times)
-    if dist is not None:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    h2d = h_reads.numel() * 4 + h_mask.numel() * 4 + h_lens.numel() * 4
-    d2h = sum(v.numel() * v.element_size() for v in out.values())
-    same = bool((out["top2"] == top2.cpu()).all())
+    e2e = None
+    if args.mode == "plain":
+        out = mss.mss_map_align_host(G, h_reads, h_mask, h_lens, m, sc, cfg.strands, 30, args.cigar_stride)   # warm-up
+        e2e_times = []
+        for _ in range(max(1, min(args.steps, 2))):
+            flush.fill_(1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            out = mss.mss_map_align_host(G, h_reads, h_mask, h_lens, m, sc, cfg.strands, 30, args.cigar_stride, out=out)
+            e2e_times.append(time.perf_counter() - t0)
+        e2e_s = sum(e2e_times) / len(e2e_times)
+        if dist is not None:
+            t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        h2d = h_reads.numel() * 4 + h_mask.numel() * 4 + h_lens.numel() * 4
+        d2h = sum(v.numel() * v.element_size() for v in out.values())
+        same = bool((out["top2"] == top2.cpu()).all())
+        e2e = {"value": cells_step * world / e2e_s / 1e9, "unit": "GCUPS", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s, "matches_device_path": same,
+               "api": "mss_map_align_host (pinned host buffers in/out)"}
 
     if rank != 0:
         if dist is not None:
@@ -288,7 +314,8 @@ def main():
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "s16x2 (int16 lanes, exact)",
         "data": "synthetic",
         "config": {"workload": f"config {cfg.c} ({cfg.name}): {n_reads} reads x {m} bp per GPU vs {cfg.genome_len} bp genome, "
-                               f"F={cfg.frag_len}, overlap={'m-1' if cfg.overlap < 0 else cfg.overlap}, both strands, top-2 + NW",
+                               f"F={cfg.frag_len}, overlap={'m-1' if cfg.overlap < 0 else cfg.overlap}, both strands, top-2 + NW"
+                               + ("" if args.mode == "plain" else f" [diagnostic mode: {args.mode}]"),
                    "reads_per_gpu": n_reads, "read_len": m, "genome_bp": cfg.genome_len, "frag_len": cfg.frag_len,
                    "n_frag": G.n_frag, "l2": "flushed between steps (256 MiB write); genome (1.7 MB) is L2-resident by design",
                    "parallelism": f"reads sharded over {world} GPU(s), genome replicated, no collective",
@@ -296,10 +323,8 @@ def main():
         "reads_per_s": n_reads * world / (ms_per_step * 1e-3),
         "scan_gcups": cells_step / (scan_avg_ms * 1e-3) / 1e9, "scan_ms": scan_avg_ms, "nw_ms": sum(nw_ms) / len(nw_ms),
         "genome_load_ms": genome_load_ms,
-        "e2e": {"value": cells_step * world / e2e_s / 1e9, "unit": "GCUPS", "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s, "matches_device_path": same,
-                "api": "mss_map_align_host (pinned host buffers in/out)"},
-        "gpu_launches": args.steps * (launch_info["launches"] + (0 if args.no_nw else 1)),
+        "e2e": e2e,
+        "gpu_launches": args.steps * (launch_info["launches"] + (0 if args.no_nw else 1) + (1 if args.mode == "pssm" else 0)),
         "clocks": clocks, "roofline": roofline,
     }
     if world == 1 and not args.no_cpu_baseline:

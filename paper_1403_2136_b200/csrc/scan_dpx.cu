@@ -21,6 +21,7 @@ namespace {
 
 struct DpxUnitGeom {
     int32_t n_groups, n_splits, frags_per_split, reads_per_group;
+    int32_t nq;                      // queries (read x strand) per block: NQ_MAX, fewer for long reads (tables must fit)
 };
 
 template <int K, int T>
@@ -30,22 +31,26 @@ struct Cfg {
     static constexpr int NW = T / 32;
 };
 
-constexpr int NQ_MAX = 32;          // queries (read x strand) per block
+constexpr int NQ_MAX = 32;          // most queries (read x strand) per block
 
 __device__ __forceinline__ uint32_t pack2(int32_t lo, int32_t hi)
 {
     return ((uint32_t)lo & 0xFFFFu) | ((uint32_t)hi << 16);
 }
 
-// select per lane: mask lane 0xFFFF -> a, 0x0000 -> b (one LOP3)
-__device__ __forceinline__ uint32_t lane_select(uint32_t mask, uint32_t a, uint32_t b)
+// PSSM step: both lanes of h get += eq * d (eq = 0/1 per lane, d = pmatch - pmismatch >= 0) in one IMAD on the FMA pipe
+// (lanes never carry: h + d <= 32767 is checked on the host), then max(. + pmismatch, 0) on the DPX pipe.
+__device__ __forceinline__ uint32_t pssm_step(uint32_t h, uint32_t eq, uint32_t d, uint32_t mm, uint32_t zero)
 {
-    return (mask & a) | (~mask & b);
+    uint32_t t;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(t) : "r"(eq), "r"(d), "r"(h));
+    return __viaddmax_s16x2(t, mm, zero);
 }
 
 // PSSM = false: the two global scores are baked into the planes (the paper's "trivial match or mismatch cost").
-// PSSM = true : the planes hold equality masks and every step selects the query position's own (pmatch, pmismatch)
-//               (base-quality position-specific scoring): one extra LOP3 per 2 cells.
+// PSSM = true : the planes hold equality bits (1 / 0 per lane) and every step applies the query position's own
+//               (pmatch, pmismatch) (base-quality position-specific scoring) as
+//               H = max(H + eq*(pmatch - pmismatch) + pmismatch, 0): one extra IMAD (FMA pipe) per 2 cells.
 // p.istep = 2 (MaxSSmap_fast) only changes the tables built in a1: step j reads read position 2j.
 template <int K, int T, bool PSSM>
 __global__ void __launch_bounds__(T)
@@ -54,9 +59,9 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
     using C = Cfg<K, T>;
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t* planes = smem;                                   // 5 * ROWW
-    uint32_t* roff = planes + 5 * ROWW;                        // NQ_MAX * MP
-    uint2* pq = reinterpret_cast<uint2*>(roff + NQ_MAX * MP);  // PSSM only: NQ_MAX * MP packed (pmatch x2, pmismatch x2)
-    uint32_t* wres = roff + NQ_MAX * MP + (PSSM ? 2 * NQ_MAX * MP : 0);   // NQ_MAX * NW
+    uint32_t* roff = planes + 5 * ROWW;                        // nq * MP
+    uint2* pq = reinterpret_cast<uint2*>(roff + ug.nq * MP);   // PSSM only: nq * MP packed (pmatch x2, pmismatch x2)
+    uint32_t* wres = roff + ug.nq * MP * (PSSM ? 3 : 1);       // NQ_MAX * NW
     int32_t* qlen = (int32_t*)(wres + NQ_MAX * C::NW);         // NQ_MAX
     unsigned long long* cur = (unsigned long long*)(qlen + NQ_MAX);   // NQ_MAX (per read; 8-byte aligned by layout)
     mss_hit_t* tbest = (mss_hit_t*)(cur + NQ_MAX);             // NQ_MAX
@@ -89,8 +94,9 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
             roff[q * MP + j] = (b * (uint32_t)ROWW + col) * 4u; // byte offset into the planes
             if (PSSM) {
                 uint32_t w = live ? pssm_at(prow, m, i, strand) : 0u;      // dead steps add 0
-                uint32_t mt = w & 0xFFFFu, mm = w >> 16;
-                pq[q * MP + j] = make_uint2(mt | (mt << 16), mm | (mm << 16));
+                int32_t mt = (int32_t)(int16_t)(w & 0xFFFFu);
+                uint32_t mm = w >> 16;
+                pq[q * MP + j] = make_uint2((uint32_t)(mt - (int32_t)(int16_t)mm), mm | (mm << 16));   // (pmatch - pmismatch, pmismatch x2)
             }
         }
         if (lane == 0) qlen[q] = ok ? (m + p.istep - 1) / p.istep : 0;     // number of steps
@@ -120,7 +126,7 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
                 int64_t plo = g0 + x, phi = plo + C::HALF;
                 uint32_t lo = plo < trunc ? base_at(p.gpacked, p.gnmask, plo) : 4u;
                 uint32_t hi = phi < trunc ? base_at(p.gpacked, p.gnmask, phi) : 4u;
-                const int32_t eqv = PSSM ? -1 : p.match, nev = PSSM ? 0 : p.mismatch;
+                const int32_t eqv = PSSM ? 1 : p.match, nev = PSSM ? 0 : p.mismatch;
 #pragma unroll
                 for (uint32_t c = 0; c < 4; c++)
                     planes[c * ROWW + x] = pack2(lo == c ? eqv : nev, hi == c ? eqv : nev);
@@ -154,22 +160,22 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
 #pragma unroll
                         for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
                     } else {
-                        const uint4 s01 = *reinterpret_cast<const uint4*>(pq + q * MP + i0);        // (mt0, mm0, mt1, mm1)
+                        const uint4 s01 = *reinterpret_cast<const uint4*>(pq + q * MP + i0);        // (d0, mm0, d1, mm1)
                         const uint4 s23 = *reinterpret_cast<const uint4*>(pq + q * MP + i0 + 2);
 #pragma unroll
                         for (int k = 0; k < K; k++)
-                            Ha[k] = __viaddmax_s16x2(H[k], lane_select(*reinterpret_cast<const uint32_t*>(my + o.x + k * T * 4), s01.x, s01.y), zero);
+                            Ha[k] = pssm_step(H[k], *reinterpret_cast<const uint32_t*>(my + o.x + k * T * 4), s01.x, s01.y, zero);
 #pragma unroll
                         for (int k = 0; k < K; k++)
-                            H[k] = __viaddmax_s16x2(Ha[k], lane_select(*reinterpret_cast<const uint32_t*>(my + o.y + k * T * 4), s01.z, s01.w), zero);
+                            H[k] = pssm_step(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.y + k * T * 4), s01.z, s01.w, zero);
 #pragma unroll
                         for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
 #pragma unroll
                         for (int k = 0; k < K; k++)
-                            Ha[k] = __viaddmax_s16x2(H[k], lane_select(*reinterpret_cast<const uint32_t*>(my + o.z + k * T * 4), s23.x, s23.y), zero);
+                            Ha[k] = pssm_step(H[k], *reinterpret_cast<const uint32_t*>(my + o.z + k * T * 4), s23.x, s23.y, zero);
 #pragma unroll
                         for (int k = 0; k < K; k++)
-                            H[k] = __viaddmax_s16x2(Ha[k], lane_select(*reinterpret_cast<const uint32_t*>(my + o.w + k * T * 4), s23.z, s23.w), zero);
+                            H[k] = pssm_step(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.w + k * T * 4), s23.z, s23.w, zero);
 #pragma unroll
                         for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
                     }
@@ -253,11 +259,12 @@ __global__ void top2_merge_kernel(const mss_top2_t* __restrict__ partial, int32_
     out[r].second = second;
 }
 
-DpxUnitGeom unit_geom(const mss_genome* g, int32_t n_reads, int32_t strands)
+DpxUnitGeom unit_geom(const mss_genome* g, int32_t n_reads, int32_t strands, int32_t nq)
 {
     DpxUnitGeom ug;
     int32_t ns = strands == 3 ? 2 : 1;
-    ug.reads_per_group = NQ_MAX / ns;
+    ug.nq = nq;
+    ug.reads_per_group = nq / ns;
     ug.n_groups = (n_reads + ug.reads_per_group - 1) / ug.reads_per_group;
     if (ug.n_groups < 1) ug.n_groups = 1;
     // blocks are long (a group of reads against a whole range of fragments): aim for >= ~48 waves of 3 resident blocks
@@ -277,7 +284,7 @@ const Variant kVariants[] = { {2, 8, 256}, {3, 8, 128}, {4, 8, 64}, {5, 4, 256},
 
 // shared-memory geometry: MP = steps per query rounded to 4 (table rows), ROWW = plane columns (tile half + read length)
 struct SmemGeom { int32_t MP, ROWW; size_t bytes; };
-SmemGeom smem_geom(int half, int nw, int32_t max_len, int32_t istep, bool pssm)
+SmemGeom smem_geom(int half, int nw, int32_t max_len, int32_t istep, bool pssm, int32_t nq)
 {
     SmemGeom s;
     int32_t steps = (max_len + istep - 1) / istep;
@@ -285,7 +292,7 @@ SmemGeom smem_geom(int half, int nw, int32_t max_len, int32_t istep, bool pssm)
     int32_t MPL = (max_len + 3) & ~3;
     if (MPL < s.MP) MPL = s.MP;
     s.ROWW = (half + MPL + 3) & ~3;
-    s.bytes = (size_t)(5 * s.ROWW + NQ_MAX * s.MP * (pssm ? 3 : 1) + NQ_MAX * nw) * 4 + NQ_MAX * 4 + NQ_MAX * 8
+    s.bytes = (size_t)(5 * s.ROWW + nq * s.MP * (pssm ? 3 : 1) + NQ_MAX * nw) * 4 + NQ_MAX * 4 + NQ_MAX * 8
             + 2 * NQ_MAX * sizeof(mss_hit_t) + NQ_MAX * 4;
     return s;
 }
@@ -295,7 +302,7 @@ cudaError_t launch_variant2(const mss_genome* g, const ScanParams& p, const DpxU
                             cudaStream_t st, mss_launch_info_t* info, int id)
 {
     using C = Cfg<K, T>;
-    SmemGeom sg = smem_geom(C::HALF, C::NW, p.max_len, p.istep, PSSM);
+    SmemGeom sg = smem_geom(C::HALF, C::NW, p.max_len, p.istep, PSSM, ug.nq);
     int32_t MP = sg.MP, ROWW = sg.ROWW;
     size_t smem = sg.bytes;
     if (smem > (size_t)g->max_smem_optin) return cudaErrorInvalidConfiguration;
@@ -318,18 +325,26 @@ cudaError_t launch_variant(const mss_genome* g, const ScanParams& p, const DpxUn
                   : launch_variant2<K, T, false>(g, p, ug, partial, st, info, id);
 }
 
-bool variant_fits(const mss_genome* g, const ScanParams& p, const Variant& v)
+bool variant_fits(const mss_genome* g, const ScanParams& p, const Variant& v, int32_t nq)
 {
-    return smem_geom(v.K * v.T, v.T / 32, p.max_len, p.istep, p.pssm != nullptr).bytes <= (size_t)g->max_smem_optin;
+    return smem_geom(v.K * v.T, v.T / 32, p.max_len, p.istep, p.pssm != nullptr, nq).bytes <= (size_t)g->max_smem_optin;
 }
 
-int pick_variant(const mss_genome* g, const ScanParams& p, int requested)
+// queries per block: as many as the shared memory allows next to the smallest tile (long reads get fewer; 0 = none fits)
+int32_t pick_nq(const mss_genome* g, const ScanParams& p)
 {
-    for (const Variant& v : kVariants) if (v.id == requested && variant_fits(g, p, v)) return requested;
+    for (int32_t nq = NQ_MAX; nq >= 2; nq >>= 1)
+        if (smem_geom(512, 2, p.max_len, p.istep, p.pssm != nullptr, nq).bytes + 32 * 1024 <= (size_t)g->max_smem_optin) return nq;
+    return 0;
+}
+
+int pick_variant(const mss_genome* g, const ScanParams& p, int requested, int32_t nq)
+{
+    for (const Variant& v : kVariants) if (v.id == requested && variant_fits(g, p, v, nq)) return requested;
     // automatic: among the tiles whose shared memory fits, the one with the least padding waste (larger tiles on ties)
     int best = 4; double best_waste = 1e30;
     for (const Variant& v : kVariants) {
-        if (v.id > 4 || !variant_fits(g, p, v)) continue;        // 5, 6 are tuning variants, never automatic
+        if (v.id > 4 || !variant_fits(g, p, v, nq)) continue;        // 5, 6 are tuning variants, never automatic
         int D = 2 * v.K * v.T;
         double waste = (double)((g->frag_len + D - 1) / D) * D / g->frag_len;
         if (waste < best_waste - 1e-9) { best_waste = waste; best = v.id; }
@@ -343,23 +358,31 @@ bool scan_dpx_supported(const mss_genome* g, const ScanParams& p)
 {
     if (g->frag_len < 256) return false;                        // tiles would be mostly padding: generic kernel
     if ((int64_t)p.max_len * p.match > 32767 || p.mismatch < -32768) return false;
-    return smem_geom(512, 2, p.max_len, p.istep, p.pssm != nullptr).bytes <= (size_t)g->max_smem_optin;   // smallest tile (K8,T64)
+    // PSSM lanes hold H + (pmatch - pmismatch) before the mismatch is added back: keep that inside int16 too
+    if (p.pssm && (int64_t)p.max_len * p.match + ((int64_t)p.match - p.mismatch) > 32767) return false;
+    return pick_nq(g, p) >= 2;
 }
 
 size_t scan_dpx_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, int32_t strands)
 {
     (void)max_len;
-    DpxUnitGeom ug = unit_geom(g, n_reads > 0 ? n_reads : 1, strands);
-    return (size_t)ug.n_splits * (size_t)(n_reads > 0 ? n_reads : 1) * sizeof(mss_top2_t) + 256;
+    int32_t n = n_reads > 0 ? n_reads : 1, most = 1;
+    for (int32_t nq = NQ_MAX; nq >= 2; nq >>= 1) {               // the split count depends on the queries per block
+        int32_t sp = unit_geom(g, n, strands, nq).n_splits;
+        if (sp > most) most = sp;
+    }
+    return (size_t)most * (size_t)n * sizeof(mss_top2_t) + 256;
 }
 
 cudaError_t launch_scan_dpx(const mss_genome* g, const ScanParams& p, void* ws, size_t ws_bytes,
                             mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info, int variant)
 {
     (void)ws_bytes;
-    DpxUnitGeom ug = unit_geom(g, p.n_reads, p.strands);
+    int32_t nq = pick_nq(g, p);
+    if (nq < 2) return cudaErrorInvalidConfiguration;
+    DpxUnitGeom ug = unit_geom(g, p.n_reads, p.strands, nq);
     mss_top2_t* partial = (mss_top2_t*)ws;
-    int id = pick_variant(g, p, variant);
+    int id = pick_variant(g, p, variant, nq);
     cudaError_t e;
     switch (id) {
         case 3: e = launch_variant<8, 128>(g, p, ug, partial, st, info, id); break;

@@ -148,6 +148,28 @@ def test_long_reads_up_to_the_s16_limit(oracle_mod, m):
     reads[0] = g[1000:1000 + m]                                                 # exact read: score m*match, the s16 extreme
     want = _both(oracle_mod, g, 8192, -1, reads, r["lens"], variants=(0,))
     assert want[0, 0].tolist() == [0, 1000, 5 * m, 0]
+    import paper_1403_2136_b200 as mss
+    info = mss.mss_get_last_launch()
+    assert info["variant"] != 1, info           # the tile kernel (fewer reads per block), not the generic fallback
+
+
+def test_long_reads_several_groups_all_modes(oracle_mod):
+    """m = 1500: 16 queries per block instead of 32, so 11 reads span two read groups; plain, fast and PSSM scans."""
+    from gpu_util import load_genome, map_reads, map_reads_fast, map_reads_pssm, pssm_tables
+    m, n = 1500, 11
+    g = gen.make_genome(30_000, 21)[0]
+    r = gen.make_reads(g, n, m, 2100, sub_rate=0.1, indel_counts=(0, 1, 2))
+    reads, lens = r["reads"], r["lens"].copy()
+    lens[3], lens[7] = 1499, 801
+    reads[3, 1499:] = gen.N
+    reads[7, 801:] = gen.N
+    G = load_genome(g, 4096, -1)
+    _cmp(map_reads(G, reads, lens), oracle_mod.map_reads_parallel(g, 4096, -1, reads, lens, strands=3), "plain m=1500")
+    _cmp(map_reads_fast(G, reads, lens), oracle_mod.map_reads_parallel(g, 4096, -1, reads, lens, strands=3, fast=True), "fast m=1500")
+    quals = gen.make_quals(n, m, 2101)
+    d_pssm, pm, pmm = pssm_tables(quals, lens, scale=4)
+    _cmp(map_reads_pssm(G, reads, lens, d_pssm, scale=4),
+         oracle_mod.map_reads_pssm_parallel(g, 4096, -1, reads, lens, pm, pmm, strands=3), "pssm m=1500")
 
 
 def test_other_scorings_and_range_errors(oracle_mod):
