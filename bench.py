@@ -27,6 +27,7 @@ sys.path.insert(0, ROOT)
 import gen  # noqa: E402
 
 ALGO_INSTR_PER_CELL = 0.75          # 1 VIADDMNMX.S16x2 per 2 cells + 1 VIMNMX3.S16x2 per 4 cells
+NCU_DRAM_BYTES_PER_LAUNCH = 2_043_648   # profiles/r1_scan_dpx_full.md (2.04 MB read + 0 written per launch)
 ALU_LANES_PER_CLK_SM = 64           # integer/DPX pipe: 16 lanes/clk per SM sub-partition x 4 (guide + measured)
 
 
@@ -303,7 +304,9 @@ def main():
     achieved = cells_step * ALGO_INSTR_PER_CELL / (scan_avg_ms * 1e-3)
     probe_rate, _ = mss.mss_probe_dpx_peak(2048)
     roofline = {"bound": "alu", "kernel": "scan_dpx_kernel", "achieved": achieved / 1e12, "peak": peak_instr / 1e12,
-                "unit": "T thread-instr/s", "frac": achieved / peak_instr, "traffic": None,
+                "unit": "T thread-instr/s", "frac": achieved / peak_instr, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1_scan_dpx_full.md (ncu --set full, one "
+                                  "4096-read launch of this kernel: the 1.7 MB genome once, then L2)",
                 "peak_source": f"{n_sm} SMs x {ALU_LANES_PER_CLK_SM} lanes/clk x {sm_max:.0f} MHz (clocks.max.sm of MEASURED_PEAKS.json)",
                 "algorithmic_instr_per_cell": ALGO_INSTR_PER_CELL, "cells_per_launch": cells_step,
                 "kernel_ms": scan_avg_ms, "probe_dpx_peak": probe_rate / 1e12,
