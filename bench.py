@@ -80,7 +80,7 @@ def cpu_baseline(cfg, genome, reads, lens, target_s: float = 15.0) -> dict:
     oracle.build()
     cores = os.cpu_count() or 1
     per_read_cells = cfg.cells() / cfg.n_reads
-    guess = 0.55e9                                   # cells/s/core of the plain -O3 build (measured in DESIGN.md)
+    guess = 1.4e9                                    # cells/s/core of the plain -O3 build (measured in DESIGN.md)
     per_core = max(1, int(target_s * guess / per_read_cells))
     n = min(reads.shape[0], cores * per_core)
     t0 = time.perf_counter()
