@@ -52,21 +52,29 @@ def sha256_of(*arrays: np.ndarray) -> str:
 
 # ----------------------------------------------------------------------------- wire format
 
+_PACK_CHUNK = 1 << 26      # bases per packing chunk (multiple of 32): bounds the temporaries for Gbp-sized genomes
+
+
 def pack_2bit(codes: np.ndarray, n_words: int | None = None):
     """codes (uint8, 0..4) -> (packed uint32[ceil(n/16)], nmask uint32[ceil(n/32)])."""
     codes = np.asarray(codes, dtype=np.uint8).ravel()
     n = codes.size
     nw = (n + 15) // 16 if n_words is None else n_words
-    pad = np.zeros(nw * 16, dtype=np.uint8)
-    pad[:n] = np.where(codes < 4, codes, 0)
-    q = pad.reshape(nw, 16).astype(np.uint32)
-    shifts = (2 * np.arange(16, dtype=np.uint32))[None, :]
-    packed = np.bitwise_or.reduce(q << shifts, axis=1).astype(np.uint32)
     nmw = (nw * 16 + 31) // 32
-    isn = np.zeros(nmw * 32, dtype=np.uint8)
-    isn[:n] = codes >= 4
-    b = isn.reshape(nmw, 32).astype(np.uint32)
-    nmask = np.bitwise_or.reduce(b << np.arange(32, dtype=np.uint32)[None, :], axis=1).astype(np.uint32)
+    packed = np.zeros(nw, dtype=np.uint32)
+    nmask = np.zeros(nmw, dtype=np.uint32)
+    shifts = (2 * np.arange(16, dtype=np.uint32))[None, :]
+    mshifts = np.arange(32, dtype=np.uint32)[None, :]
+    for c0 in range(0, max(n, 1), _PACK_CHUNK):
+        part = codes[c0:c0 + _PACK_CHUNK]
+        k = part.size
+        kw, km = (k + 15) // 16, (k + 31) // 32
+        pad = np.zeros(kw * 16, dtype=np.uint8)
+        pad[:k] = np.where(part < 4, part, 0)
+        packed[c0 // 16:c0 // 16 + kw] = np.bitwise_or.reduce(pad.reshape(kw, 16).astype(np.uint32) << shifts, axis=1)
+        isn = np.zeros(km * 32, dtype=np.uint8)
+        isn[:k] = part >= 4
+        nmask[c0 // 32:c0 // 32 + km] = np.bitwise_or.reduce(isn.reshape(km, 32).astype(np.uint32) << mshifts, axis=1)
     return packed, nmask
 
 
@@ -129,8 +137,14 @@ def make_genome(n: int, seed: int, gc: float = 0.5, dup_frac: float = 0.0, n_fra
     rng = np.random.Generator(np.random.PCG64(seed))
     p = np.array([(1 - gc) / 2, gc / 2, gc / 2, (1 - gc) / 2])
     cdf = np.cumsum(p)
-    g = np.searchsorted(cdf, rng.random(n, dtype=np.float32), side="right").astype(np.uint8)
-    g = np.minimum(g, 3).astype(np.uint8)
+    if n <= _PACK_CHUNK * 16:
+        g = np.searchsorted(cdf, rng.random(n, dtype=np.float32), side="right").astype(np.uint8)
+        g = np.minimum(g, 3).astype(np.uint8)
+    else:           # Gbp-sized genomes (config 6): the same draw rule chunk by chunk, to bound the temporaries
+        g = np.empty(n, dtype=np.uint8)
+        for c0 in range(0, n, _PACK_CHUNK):
+            k = min(_PACK_CHUNK, n - c0)
+            g[c0:c0 + k] = np.minimum(np.searchsorted(cdf, rng.random(k, dtype=np.float32), side="right"), 3)
     info = {"dups": [], "n_runs": []}
     occupied = np.zeros(n, dtype=bool)
     if dup_frac > 0:
@@ -339,6 +353,9 @@ CONFIGS = {
     4: Config(4, "chr1", 249_000_000, 16384, -1, 3, gc=0.41, dup_frac=0.02, n_frac=0.10,
               groups=((10_000, 150, 0.20),), avoid_n=True),
     5: Config(5, "throughput", 4_600_000, 4096, -1, 3, genome_of=2, groups=((1_000_000, 100, 0.30),)),
+    # next-4: whole-genome-sized workload in the shape of the paper's Table 8 (PAPER.md:460-474, :182:
+    # 100k x 76 bp reads against the 2.4 Gbp horse genome, fragment length 4800): the packed genome (0.9 GB) no longer fits L2
+    6: Config(6, "wholegenome", 2_400_000_000, 4800, -1, 3, gc=0.41, groups=((100_000, 76, 0.20),)),
 }
 
 

@@ -33,6 +33,8 @@ def main():
     ap.add_argument("--mode", default="plain", choices=["plain", "fast", "pssm"])
     ap.add_argument("--nw-reads", type=int, default=4096, help="reads whose second stage is also compared (evenly spaced)")
     ap.add_argument("--chunk", type=int, default=2048)
+    ap.add_argument("--workers", type=int, default=None,
+                    help="oracle processes (default: every host core; each holds its own copy of the genome, so use few for Gbp genomes)")
     ap.add_argument("--out", default=None)
     args = ap.parse_args()
 
@@ -74,7 +76,7 @@ def main():
                                    nw[3].cpu().numpy())
     info = mss.mss_get_last_launch()
 
-    cores = os.cpu_count() or 1
+    cores = args.workers or os.cpu_count() or 1
     bad_top2, checked = [], 0
     t0 = time.perf_counter()
     want_all = np.zeros_like(got)
