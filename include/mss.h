@@ -231,13 +231,29 @@ int mss_last_cuda_error(void);                 /* cudaError_t of the last MSS_ER
 int mss_version(void);                         /* 100*major + minor */
 
 /*
- * Tuning / introspection (does not change results): select the scan kernel variant (0 = automatic) and report the
+ * Tuning / introspection (does not change results): select the scan kernel variant (0 = automatic: the two-pass scan
+ * where the geometry allows it, else the one-pass tile kernel, else the generic kernel; 1 = generic; 2-6 = one-pass tile
+ * kernels (K, T) = (8,256), (8,128), (8,64), (4,256), (16,128); 7 = two-pass, same as automatic) and report the
  * launch geometry of the last mss_map_reads call on this thread.  Used by bench.py and the parity tests to cover
  * every variant.
  */
 int mss_set_scan_variant(int variant);
 typedef struct { int32_t variant, grid, block, smem_bytes, reads_per_block, tile_diagonals, launches; } mss_launch_info_t;
 int mss_get_last_launch(mss_launch_info_t *out);
+
+/*
+ * Pass 1 of the two-pass scan on its own (scan variant 7): for every read, enabled strand and fragment
+ * a 16-bit lower bound u of the fragment's exact MaxSS score with  u <= score <= u + *h_delta  (two Kadane steps per
+ * DPX instruction, H sampled after every second step), or 0xFFFF = "not bounded" (reads holding an N, bad lengths).
+ * d_bounds holds n_reads * (strands == MSS_BOTH ? 2 : 1) * n_fragments uint16, indexed [read][strand][fragment];
+ * every_other != 0 bounds the MaxSSmap_fast scores instead.  MSS_ERR_RANGE if the geometry has no two-pass path
+ * (fewer than 8 fragments, frag_len < 256, 2*match or 2*mismatch outside int16).  mss_map_reads itself uses these
+ * bounds only to skip fragments that cannot reach a read's top-2; its records are those of the one-pass scan.
+ */
+int mss_map_reads_bounds(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
+                         int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
+                         mss_scoring_t sc, int32_t strands, int32_t every_other, void *stream,
+                         uint16_t *d_bounds, int32_t *h_delta);
 
 /*
  * Live measurement of the integer/DPX issue peak the scan's roofline is quoted against: runs `iters` dependent

@@ -80,6 +80,8 @@ def lib() -> C.CDLL:
     L.mss_nw_align.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, _Scoring, i32, vp, sz, vp, vp, vp, vp, i32, vp]
     L.mss_nw_align.restype = C.c_int
     L.mss_mapq_filter.argtypes = [vp, i32, C.c_float, vp, vp, vp]; L.mss_mapq_filter.restype = C.c_int
+    L.mss_map_reads_bounds.argtypes = [vp, vp, vp, i32, vp, i32, i32, _Scoring, i32, i32, vp, vp, C.POINTER(i32)]
+    L.mss_map_reads_bounds.restype = C.c_int
     L.mss_map_reads_fast.argtypes = L.mss_map_reads.argtypes; L.mss_map_reads_fast.restype = C.c_int
     L.mss_pssm_build.argtypes = [vp, i32, vp, i32, _Scoring, i32, vp, vp, i32]; L.mss_pssm_build.restype = C.c_int
     L.mss_map_reads_pssm.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, i32, _Scoring, i32, vp, sz, vp, vp]
@@ -207,6 +209,21 @@ def mss_map_reads_fast(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, 
     _check(L.mss_map_reads_fast(g.handle, _ptr(d_reads), _ptr(d_reads_nmask), stride, _ptr(d_lens), n, max_len, scoring.c(),
                                 strands, _ptr(ws), ws.numel(), _stream(stream), _ptr(out)), "mss_map_reads_fast")
     return out
+
+
+def mss_map_reads_bounds(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, scoring: Scoring = Scoring(),
+                         strands: int = MSS_BOTH, every_other: bool = False, stream=None):
+    """Pass 1 of the two-pass scan: -> (CUDA int16 tensor (n_reads, n_strands, n_frag) holding uint16 bounds, delta)."""
+    torch = _torch()
+    n = int(d_lens.numel())
+    stride = int(d_reads.shape[1])
+    ns = 2 if strands == MSS_BOTH else 1
+    out = torch.empty((n, ns, g.n_frag), dtype=torch.int16, device=d_lens.device)
+    delta = C.c_int32()
+    _check(lib().mss_map_reads_bounds(g.handle, _ptr(d_reads), _ptr(d_reads_nmask), stride, _ptr(d_lens), n, max_len,
+                                      scoring.c(), strands, 1 if every_other else 0, _stream(stream), _ptr(out),
+                                      C.byref(delta)), "mss_map_reads_bounds")
+    return out, delta.value
 
 
 def pssm_bound(scoring: Scoring, scale: int) -> Scoring:

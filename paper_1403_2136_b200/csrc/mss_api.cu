@@ -81,7 +81,9 @@ size_t mss_map_workspace_bytes(const mss_genome_t* g, int32_t n_reads, int32_t m
     if (!g || n_reads < 0 || max_len < 1 || strands < 1 || strands > 3) return 0;
     size_t a = scan_generic_workspace(g, n_reads);
     size_t b = scan_dpx_workspace(g, n_reads, max_len, strands);
-    return a > b ? a : b;
+    size_t c = scan_two_pass_workspace(g, n_reads, strands);
+    if (b > a) a = b;
+    return c > a ? c : a;
 }
 
 static int map_reads_impl(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
@@ -101,10 +103,12 @@ static int map_reads_impl(const mss_genome_t* g, const uint32_t* d_reads, const 
     p.F = g->frag_len; p.V = g->overlap; p.n_frag = g->n_frag;
     p.reads = d_reads; p.reads_nmask = d_reads_nmask; p.stride_words = read_stride_words; p.lens = d_lens;
     p.n_reads = n_reads; p.max_len = max_len; p.match = sc.match; p.mismatch = sc.mismatch; p.strands = strands; p.zero = 0;
-    p.istep = istep; p.pssm = d_pssm; p.pssm_stride = pssm_stride;
+    p.istep = istep; p.pssm = d_pssm; p.pssm_stride = pssm_stride; p.ubound = nullptr; p.delta = 0;
     cudaError_t e;
     bool use_generic = (t_variant == 1) || !scan_dpx_supported(g, p);
+    bool two_pass = !use_generic && (t_variant == 0 || t_variant == 7) && scan_filter_supported(g, p);   // 2..6: one-pass tiles
     if (use_generic) e = launch_scan_generic(g, p, d_workspace, workspace_bytes, d_out, (cudaStream_t)stream, &t_info);
+    else if (two_pass) e = launch_scan_two_pass(g, p, d_workspace, workspace_bytes, d_out, (cudaStream_t)stream, &t_info);
     else e = launch_scan_dpx(g, p, d_workspace, workspace_bytes, d_out, (cudaStream_t)stream, &t_info, t_variant);
     if (e != cudaSuccess) return cuda_fail(e);
     return MSS_OK;
@@ -124,6 +128,30 @@ int mss_map_reads_fast(const mss_genome_t* g, const uint32_t* d_reads, const uin
 {
     return map_reads_impl(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, sc, strands, d_workspace,
                           workspace_bytes, stream, d_out, 2, nullptr, 0);
+}
+
+int mss_map_reads_bounds(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                         const int32_t* d_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands,
+                         int32_t every_other, void* stream, uint16_t* d_bounds, int32_t* h_delta)
+{
+    if (!g || n_reads < 0 || strands < 1 || strands > 3 || max_len < 1) return MSS_ERR_ARG;
+    if (h_delta) *h_delta = 0;
+    if (n_reads == 0) return MSS_OK;
+    if (!d_reads || !d_lens || !d_bounds) return MSS_ERR_ARG;
+    if ((int64_t)read_stride_words * 16 < max_len) return MSS_ERR_ARG;
+    int rc = check_scoring_scan(sc, max_len);
+    if (rc != MSS_OK) return rc;
+    ScanParams p;
+    p.gpacked = g->packed; p.gnmask = g->nmask; p.n_bases = g->n_bases;
+    p.F = g->frag_len; p.V = g->overlap; p.n_frag = g->n_frag;
+    p.reads = d_reads; p.reads_nmask = d_reads_nmask; p.stride_words = read_stride_words; p.lens = d_lens;
+    p.n_reads = n_reads; p.max_len = max_len; p.match = sc.match; p.mismatch = sc.mismatch; p.strands = strands; p.zero = 0;
+    p.istep = every_other ? 2 : 1; p.pssm = nullptr; p.pssm_stride = 0; p.ubound = nullptr; p.delta = 0;
+    if (!scan_filter_supported(g, p)) return MSS_ERR_RANGE;
+    if (h_delta) *h_delta = scan_filter_delta(p);
+    cudaError_t e = launch_scan_filter(g, p, d_bounds, (cudaStream_t)stream, nullptr, nullptr, nullptr);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return MSS_OK;
 }
 
 int mss_pssm_build(const uint8_t* d_qual, int32_t qual_stride, const int32_t* d_lens, int32_t n_reads, mss_scoring_t sc,

@@ -38,6 +38,8 @@ struct ScanParams {
     int32_t istep;                 // 1 = every read position; 2 = MaxSSmap_fast, every other position
     const uint32_t* pssm;          // nullable: per-read rows of (int16 pmatch | int16 pmismatch << 16) per position
     int32_t pssm_stride;           // words per row of pssm
+    const uint16_t* ubound;        // nullable: pass-1 fragment score bounds [read][strand][fragment] (two-pass scan, pass 2)
+    int32_t delta;                 // bound slack: a fragment's exact score lies in [ubound, ubound + delta]
 };
 
 // candidate of one fragment for one read: higher key = better under (score desc, strand asc, diag asc)
@@ -107,6 +109,15 @@ __device__ __forceinline__ uint32_t pssm_at(const uint32_t* row, int32_t m, int3
 }
 cudaError_t launch_scan_dpx(const mss_genome* g, const ScanParams& p, void* ws, size_t ws_bytes,
                             mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info, int variant);
+
+// two-pass scan (scan_filter.cu): bounded-error pass 1, then the exact kernel on the candidate fragments only
+bool scan_filter_supported(const mss_genome* g, const ScanParams& p);
+int32_t scan_filter_delta(const ScanParams& p);
+cudaError_t launch_scan_filter(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
+                               int32_t* smem_out, int32_t* tile_out);
+size_t scan_two_pass_workspace(const mss_genome* g, int32_t n_reads, int32_t strands);
+cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p, void* ws, size_t ws_bytes,
+                                 mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info);
 
 size_t nw_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t pad);
 cudaError_t launch_nw(const mss_genome* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t stride_words,

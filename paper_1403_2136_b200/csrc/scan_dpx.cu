@@ -113,7 +113,48 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
     const uint32_t zero = (uint32_t)p.zero;                     // opaque 0: keeps ptxas from re-materialising it per use
     const int32_t tiles_per_frag = (p.F + C::D - 1) / C::D;
 
+    // ---- two-pass scan, pass 2 (one read per block): the lower bound L2 of the read's second-best fragment score ----
+    // Pass 1 left u = ubound[read][strand][f] with u <= exact <= u + delta (0xFFFF = unknown).  Two fragments score at
+    // least L2 = the second largest max-over-strands u, so a fragment with u + delta < L2 lies strictly below the
+    // read's second place and can never enter its top-2 (a5 replaces on strictly greater): it is skipped.
+    __shared__ int32_t s_top[2 * 32];
+    __shared__ int32_t s_l2;
+    const uint16_t* ub0 = nullptr;
+    if (p.ubound) {
+        ub0 = p.ubound + (int64_t)r0 * ns * p.n_frag;
+        int32_t v1 = 0, v2 = 0;
+        for (int32_t f = tid; f < p.n_frag; f += T) {
+            int32_t u = ub0[f];
+            if (ns == 2) u = max(u, (int32_t)ub0[p.n_frag + f]);
+            if (u == 0xFFFF) u = 0;                             // unknown: no information for the lower bound
+            if (u > v1) { v2 = v1; v1 = u; } else if (u > v2) v2 = u;
+        }
+        for (int off = 16; off; off >>= 1) {                    // warp top-2 (values of distinct fragments)
+            int32_t o1 = __shfl_xor_sync(0xffffffffu, v1, off), o2 = __shfl_xor_sync(0xffffffffu, v2, off);
+            int32_t n1 = max(v1, o1), n2 = max(min(v1, o1), max(v2, o2));
+            v1 = n1; v2 = n2;
+        }
+        if (lane == 0) { s_top[2 * warp] = v1; s_top[2 * warp + 1] = v2; }
+        __syncthreads();
+        if (tid == 0) {
+            int32_t a = 0, b = 0;
+            for (int w = 0; w < C::NW; w++) {
+                int32_t x1 = s_top[2 * w], x2 = s_top[2 * w + 1];
+                int32_t n1 = max(a, x1), n2 = max(min(a, x1), max(b, x2));
+                a = n1; b = n2;
+            }
+            s_l2 = b;
+        }
+        __syncthreads();
+    }
+    const int32_t l2 = p.ubound ? s_l2 : 0;
+
     for (int32_t f = f_begin; f < f_end; f++) {
+        if (ub0) {                                              // block-uniform: every thread reads the same two values
+            int32_t u = ub0[f];
+            if (ns == 2) u = max(u, (int32_t)ub0[p.n_frag + f]);
+            if (u != 0xFFFF && u + p.delta < l2) continue;
+        }
         const int64_t fstart = (int64_t)f * p.F;
         const int64_t trunc = (p.V < 0) ? (int64_t)0x7FFFFFFFFFFFFFFFll : fstart + p.F + p.V;   // positions >= trunc are not readable
         for (int32_t tile = 0; tile < tiles_per_frag; tile++) {
@@ -394,4 +435,63 @@ cudaError_t launch_scan_dpx(const mss_genome* g, const ScanParams& p, void* ws, 
     if (e != cudaSuccess) return e;
     top2_merge_kernel<<<(p.n_reads + 255) / 256, 256, 0, st>>>(partial, ug.n_splits, p.n_reads, d_out);
     return cudaGetLastError();
+}
+
+// ---- two-pass scan: bounded-error pass 1 (scan_filter.cu), exact pass 2 on the candidate fragments ----
+namespace {
+int32_t two_pass_chunk(const mss_genome* g, int32_t n_reads, int32_t strands)
+{
+    int64_t per_read = (int64_t)(strands == 3 ? 2 : 1) * g->n_frag * 2;         // bytes of bounds per read
+    int64_t c = (1ll << 30) / per_read;
+    if (c < 1) c = 1;
+    if (c > n_reads) c = n_reads;
+    if (c < 1) c = 1;
+    return (int32_t)c;
+}
+}  // namespace
+
+size_t scan_two_pass_workspace(const mss_genome* g, int32_t n_reads, int32_t strands)
+{
+    int32_t n = n_reads > 0 ? n_reads : 1;
+    return (size_t)two_pass_chunk(g, n, strands) * (size_t)(strands == 3 ? 2 : 1) * (size_t)g->n_frag * 2 + 256;
+}
+
+cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void* ws, size_t ws_bytes,
+                                 mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info)
+{
+    (void)ws_bytes;
+    const int32_t ns = p0.strands == 3 ? 2 : 1;
+    const int32_t chunk = two_pass_chunk(g, p0.n_reads, p0.strands);
+    uint16_t* ubound = (uint16_t*)ws;
+    int launches = 0;
+    int32_t fgrid = 0, fsmem = 0, ftile = 0;
+    for (int32_t c0 = 0; c0 < p0.n_reads; c0 += chunk) {
+        ScanParams p = p0;
+        p.n_reads = p0.n_reads - c0 < chunk ? p0.n_reads - c0 : chunk;
+        p.reads = p0.reads + (int64_t)c0 * p0.stride_words;
+        p.reads_nmask = p0.reads_nmask ? p0.reads_nmask + (int64_t)c0 * ((p0.stride_words + 1) / 2) : nullptr;
+        p.lens = p0.lens + c0;
+        p.ubound = nullptr;
+        cudaError_t e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile);
+        if (e != cudaSuccess) return e;
+        // pass 2: one read per block, every fragment range in one block (the bounds row decides what is scanned)
+        p.ubound = ubound;
+        p.delta = scan_filter_delta(p);
+        DpxUnitGeom ug;
+        ug.nq = ns; ug.reads_per_group = 1; ug.n_groups = p.n_reads; ug.n_splits = 1; ug.frags_per_split = g->n_frag;
+        int id = pick_variant(g, p, 0, ns);
+        mss_top2_t* out = d_out + c0;
+        switch (id) {
+            case 3: e = launch_variant<8, 128>(g, p, ug, out, st, nullptr, id); break;
+            case 4: e = launch_variant<8, 64>(g, p, ug, out, st, nullptr, id); break;
+            default: e = launch_variant<8, 256>(g, p, ug, out, st, nullptr, 2); break;
+        }
+        if (e != cudaSuccess) return e;
+        launches += 2;
+    }
+    if (info) {
+        info->variant = 7; info->grid = fgrid; info->block = 0; info->smem_bytes = fsmem;
+        info->reads_per_block = 32 / ns; info->tile_diagonals = ftile; info->launches = launches;
+    }
+    return cudaSuccess;
 }

@@ -32,6 +32,8 @@ def main():
     ap.add_argument("--reads", type=int, default=None, help="first N reads of every group (default: all)")
     ap.add_argument("--mode", default="plain", choices=["plain", "fast", "pssm"])
     ap.add_argument("--nw-reads", type=int, default=4096, help="reads whose second stage is also compared (evenly spaced)")
+    ap.add_argument("--skip", type=int, default=0, help="compare only reads [skip, n) with the oracle (the GPU still maps all)")
+    ap.add_argument("--variant", type=int, default=0, help="scan variant (0 = automatic, 7 = two-pass)")
     ap.add_argument("--chunk", type=int, default=2048)
     ap.add_argument("--workers", type=int, default=None,
                     help="oracle processes (default: every host core; each holds its own copy of the genome, so use few for Gbp genomes)")
@@ -53,6 +55,7 @@ def main():
     d_reads, d_mask, d_lens = (torch.from_numpy(rp.view(np.int32)).to(dev), torch.from_numpy(rn.view(np.int32)).to(dev),
                                torch.from_numpy(lens).to(dev))
     sc = mss.Scoring()
+    mss.mss_set_scan_variant(args.variant)
     scale = 16
     pm = pmm = None
     t0 = time.perf_counter()
@@ -80,7 +83,7 @@ def main():
     bad_top2, checked = [], 0
     t0 = time.perf_counter()
     want_all = np.zeros_like(got)
-    for a in range(0, n, args.chunk):
+    for a in range(args.skip, n, args.chunk):
         b = min(n, a + args.chunk)
         if args.mode == "pssm":
             want = oracle.map_reads_pssm_parallel(genome, cfg.frag_len, cfg.overlap, reads[a:b], lens[a:b], pm[a:b], pmm[a:b],
@@ -97,7 +100,7 @@ def main():
     cpu_s = time.perf_counter() - t0
 
     # second stage on an evenly spaced subset (the oracle's full-matrix NW is the slow part there)
-    idx = np.unique(np.linspace(0, n - 1, min(n, args.nw_reads)).astype(np.int64))
+    idx = np.unique(np.linspace(args.skip, n - 1, min(n - args.skip, args.nw_reads)).astype(np.int64))
     if args.mode == "pssm":
         ws, wp, wc, wn = oracle.nw_align_pssm(genome, cfg.frag_len, cfg.overlap, reads[idx], lens[idx], want_all[idx], pm[idx],
                                               pmm[idx], scale * sc.gap, cigar_stride=64)
@@ -114,7 +117,7 @@ def main():
     cells = float(np.sum(lens if args.mode != "fast" else -(-lens // 2))) * G.n_frag * cfg.frag_len * (2 if cfg.strands == 3 else 1)
     summary = {
         "config": cfg.c, "name": cfg.name, "mode": args.mode, "reads": int(n), "read_len_max": int(m), "n_frag": int(G.n_frag),
-        "cells": cells, "top2_compared": int(checked), "top2_mismatches": len(bad_top2), "first_bad_top2": bad_top2[:5],
+        "cells": cells, "top2_compared": int(checked - args.skip), "first_read_compared": int(args.skip), "top2_mismatches": len(bad_top2), "first_bad_top2": bad_top2[:5],
         "nw_compared": int(len(idx)), "nw_mismatches": len(bad_nw), "first_bad_nw": bad_nw[:5],
         "ties_best_eq_second": int(np.sum(got[:, 0, 2] == got[:, 1, 2])),
         "ratio_ge_0.9": int(np.sum(10 * got[:, 1, 2].astype(np.int64) >= 9 * got[:, 0, 2].astype(np.int64))),

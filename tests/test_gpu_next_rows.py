@@ -27,7 +27,7 @@ def _cmp(got, want, ctx=""):
 
 # ----------------------------------------------------------------------------- MaxSSmap_fast
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
 def test_fast_tiny_every_variant(oracle_mod, tiny, variant):
     from gpu_util import load_genome, map_reads_fast
     cfg, g, reads, lens, _ = tiny
@@ -84,7 +84,7 @@ def test_pssm_build_matches_oracle_table(oracle_mod, tiny):
             assert (pm[r, lens[r]:] == 0).all() and (pmm[r, lens[r]:] == 0).all()
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
 def test_pssm_tiny_every_variant(oracle_mod, tiny, variant):
     from gpu_util import load_genome, map_reads_pssm, pssm_tables
     cfg, g, reads, lens, quals = tiny

@@ -19,7 +19,7 @@ def _cmp(got, want, ctx=""):
     assert bad.size == 0, f"{ctx}: {bad.size} reads differ, first {bad[0]}: got {got[bad[0]].tolist()} want {want[bad[0]].tolist()}"
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
 def test_tiny_config_every_variant(oracle_mod, tiny, variant):
     from gpu_util import load_genome, map_reads
     cfg, g, r = tiny
