@@ -242,6 +242,15 @@ typedef struct { int32_t variant, grid, block, smem_bytes, reads_per_block, tile
 int mss_get_last_launch(mss_launch_info_t *out);
 
 /*
+ * Per-pass device times of the two-pass scan, for the roofline of bench.py: after mss_set_pass_timing(1) every
+ * mss_map_reads / mss_map_reads_fast call on this thread that takes the two-pass path records CUDA events on its stream
+ * before pass 1, between the passes and after pass 2 (per chunk of reads); mss_get_pass_times waits for the last event
+ * of the latest such call and returns the summed milliseconds (0, 0 if that call took another path).
+ */
+int mss_set_pass_timing(int on);
+int mss_get_pass_times(float *h_pass1_ms, float *h_pass2_ms);
+
+/*
  * Pass 1 of the two-pass scan on its own (scan variant 7): for every read, enabled strand and fragment
  * a 16-bit lower bound u of the fragment's exact MaxSS score with  u <= score <= u + *h_delta  (two Kadane steps per
  * DPX instruction, H sampled after every second step), or 0xFFFF = "not bounded" (reads holding an N, bad lengths).

@@ -80,6 +80,8 @@ def lib() -> C.CDLL:
     L.mss_nw_align.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, _Scoring, i32, vp, sz, vp, vp, vp, vp, i32, vp]
     L.mss_nw_align.restype = C.c_int
     L.mss_mapq_filter.argtypes = [vp, i32, C.c_float, vp, vp, vp]; L.mss_mapq_filter.restype = C.c_int
+    L.mss_set_pass_timing.argtypes = [C.c_int]; L.mss_set_pass_timing.restype = C.c_int
+    L.mss_get_pass_times.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]; L.mss_get_pass_times.restype = C.c_int
     L.mss_map_reads_bounds.argtypes = [vp, vp, vp, i32, vp, i32, i32, _Scoring, i32, i32, vp, vp, C.POINTER(i32)]
     L.mss_map_reads_bounds.restype = C.c_int
     L.mss_map_reads_fast.argtypes = L.mss_map_reads.argtypes; L.mss_map_reads_fast.restype = C.c_int
@@ -360,6 +362,17 @@ def mss_mapq_filter(d_hits, mapq_threshold: float = 15.2, stream=None):
     _check(lib().mss_mapq_filter(_ptr(d_hits), n, float(mapq_threshold), _stream(stream), _ptr(mapped), _ptr(mapq)),
            "mss_mapq_filter")
     return mapped, mapq
+
+
+def mss_set_pass_timing(on: bool) -> None:
+    _check(lib().mss_set_pass_timing(1 if on else 0), "mss_set_pass_timing")
+
+
+def mss_get_pass_times():
+    """-> (pass 1 ms, pass 2 ms) of the latest two-pass scan on this thread (waits for it)."""
+    a, b = C.c_float(), C.c_float()
+    _check(lib().mss_get_pass_times(C.byref(a), C.byref(b)), "mss_get_pass_times")
+    return a.value, b.value
 
 
 def mss_set_scan_variant(variant: int) -> None:

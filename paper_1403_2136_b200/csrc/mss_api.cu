@@ -371,6 +371,16 @@ int mss_set_scan_variant(int variant)
     return MSS_OK;
 }
 
+int mss_set_pass_timing(int on) { scan_set_pass_timing(on != 0); return MSS_OK; }
+
+int mss_get_pass_times(float* h_pass1_ms, float* h_pass2_ms)
+{
+    if (!h_pass1_ms || !h_pass2_ms) return MSS_ERR_ARG;
+    cudaError_t e = scan_get_pass_times(h_pass1_ms, h_pass2_ms);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return MSS_OK;
+}
+
 int mss_get_last_launch(mss_launch_info_t* out)
 {
     if (!out) return MSS_ERR_ARG;

@@ -119,6 +119,9 @@ size_t scan_two_pass_workspace(const mss_genome* g, int32_t n_reads, int32_t str
 cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p, void* ws, size_t ws_bytes,
                                  mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info);
 
+void scan_set_pass_timing(bool on);
+cudaError_t scan_get_pass_times(float* pass1_ms, float* pass2_ms);
+
 size_t nw_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t pad);
 cudaError_t launch_nw(const mss_genome* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t stride_words,
                       const int32_t* d_lens, int32_t n_reads, int32_t max_len, const mss_top2_t* d_hits,

@@ -15,6 +15,7 @@
 //   per tile:  fold the per-warp slots into the read's running fragment candidate (score desc, strand asc, diag asc);
 //              at the last tile of a fragment push it into the read's top-2 (a5, strictly greater, fragments ascending)
 //   at end:    a6 emit the read's top-2 (or the unit's partial top-2, merged by top2_merge_kernel)
+#include <vector>
 #include "mss_common.cuh"
 
 namespace {
@@ -439,6 +440,22 @@ cudaError_t launch_scan_dpx(const mss_genome* g, const ScanParams& p, void* ws, 
 
 // ---- two-pass scan: bounded-error pass 1 (scan_filter.cu), exact pass 2 on the candidate fragments ----
 namespace {
+// optional CUDA-event timing of the two passes on the launching stream (mss_set_pass_timing / mss_get_pass_times)
+thread_local bool t_time_passes = false;
+thread_local std::vector<cudaEvent_t>* t_events = nullptr;      // 3 per chunk: before pass 1, between, after pass 2
+thread_local int t_events_used = 0;
+
+cudaEvent_t next_event()
+{
+    if (!t_events) t_events = new std::vector<cudaEvent_t>();
+    if (t_events_used == (int)t_events->size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+        t_events->push_back(e);
+    }
+    return (*t_events)[t_events_used++];
+}
+
 int32_t two_pass_chunk(const mss_genome* g, int32_t n_reads, int32_t strands)
 {
     int64_t per_read = (int64_t)(strands == 3 ? 2 : 1) * g->n_frag * 2;         // bytes of bounds per read
@@ -465,7 +482,11 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
     uint16_t* ubound = (uint16_t*)ws;
     int launches = 0;
     int32_t fgrid = 0, fsmem = 0, ftile = 0;
+    t_events_used = 0;
     for (int32_t c0 = 0; c0 < p0.n_reads; c0 += chunk) {
+        cudaEvent_t ev0 = t_time_passes ? next_event() : nullptr, ev1 = t_time_passes ? next_event() : nullptr,
+                    ev2 = t_time_passes ? next_event() : nullptr;
+        if (ev0) cudaEventRecord(ev0, st);
         ScanParams p = p0;
         p.n_reads = p0.n_reads - c0 < chunk ? p0.n_reads - c0 : chunk;
         p.reads = p0.reads + (int64_t)c0 * p0.stride_words;
@@ -474,6 +495,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
         p.ubound = nullptr;
         cudaError_t e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile);
         if (e != cudaSuccess) return e;
+        if (ev1) cudaEventRecord(ev1, st);
         // pass 2: one read per block, every fragment range in one block (the bounds row decides what is scanned)
         p.ubound = ubound;
         p.delta = scan_filter_delta(p);
@@ -487,6 +509,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
             default: e = launch_variant<8, 256>(g, p, ug, out, st, nullptr, 2); break;
         }
         if (e != cudaSuccess) return e;
+        if (ev2) cudaEventRecord(ev2, st);
         launches += 2;
     }
     if (info) {
@@ -494,4 +517,21 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
         info->reads_per_block = 32 / ns; info->tile_diagonals = ftile; info->launches = launches;
     }
     return cudaSuccess;
+}
+
+void scan_set_pass_timing(bool on) { t_time_passes = on; if (!on) t_events_used = 0; }
+
+// sums over the chunks of the last two-pass call on this thread; synchronises on its last event
+cudaError_t scan_get_pass_times(float* pass1_ms, float* pass2_ms)
+{
+    *pass1_ms = 0.f; *pass2_ms = 0.f;
+    if (!t_events || t_events_used < 3) return cudaSuccess;
+    cudaError_t e = cudaEventSynchronize((*t_events)[t_events_used - 1]);
+    for (int i = 0; e == cudaSuccess && i + 2 < t_events_used; i += 3) {
+        float a = 0.f, b = 0.f;
+        e = cudaEventElapsedTime(&a, (*t_events)[i], (*t_events)[i + 1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&b, (*t_events)[i + 1], (*t_events)[i + 2]);
+        *pass1_ms += a; *pass2_ms += b;
+    }
+    return e;
 }
