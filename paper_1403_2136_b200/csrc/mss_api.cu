@@ -367,6 +367,9 @@ int mss_version(void) { return 100; }
 int mss_set_scan_variant(int variant)
 {
     if (variant < 0 || variant > 16) return MSS_ERR_ARG;
+    // 8..12: the two-pass scan with one pass-1 tile geometry forced (tuning); otherwise pass 1 picks its own
+    scan_filter_force_variant(variant >= 8 && variant <= 12 ? variant - 8 : -1);
+    if (variant >= 8 && variant <= 12) variant = 7;
     t_variant = variant;
     return MSS_OK;
 }

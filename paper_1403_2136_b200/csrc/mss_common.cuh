@@ -113,6 +113,7 @@ cudaError_t launch_scan_dpx(const mss_genome* g, const ScanParams& p, void* ws, 
 // two-pass scan (scan_filter.cu): bounded-error pass 1, then the exact kernel on the candidate fragments only
 bool scan_filter_supported(const mss_genome* g, const ScanParams& p);
 int32_t scan_filter_delta(const ScanParams& p);
+void scan_filter_force_variant(int v);
 cudaError_t launch_scan_filter(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
                                int32_t* smem_out, int32_t* tile_out);
 size_t scan_two_pass_workspace(const mss_genome* g, int32_t n_reads, int32_t strands);

@@ -151,10 +151,17 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
     const int32_t l2 = p.ubound ? s_l2 : 0;
 
     for (int32_t f = f_begin; f < f_end; f++) {
+        uint32_t skipq = 0u;                                    // pass 2: strands of this fragment that cannot matter
         if (ub0) {                                              // block-uniform: every thread reads the same two values
-            int32_t u = ub0[f];
-            if (ns == 2) u = max(u, (int32_t)ub0[p.n_frag + f]);
+            int32_t u0 = ub0[f], u1 = (ns == 2) ? (int32_t)ub0[p.n_frag + f] : 0;
+            int32_t u = max(u0, u1);
             if (u != 0xFFFF && u + p.delta < l2) continue;
+            // a strand whose own bound stays below L2 scores below the read's second place: whatever it would report
+            // cannot be the score that puts this fragment into the top-2, so the other strand alone represents it
+            if (ns == 2 && u != 0xFFFF) {
+                if (u0 + p.delta < l2) skipq |= 1u;
+                if (u1 + p.delta < l2) skipq |= 2u;
+            }
         }
         const int64_t fstart = (int64_t)f * p.F;
         const int64_t trunc = (p.V < 0) ? (int64_t)0x7FFFFFFFFFFFFFFFll : fstart + p.F + p.V;   // positions >= trunc are not readable
@@ -179,7 +186,7 @@ scan_dpx_kernel(ScanParams p, DpxUnitGeom ug, int32_t MP, int32_t ROWW, mss_top2
             // ---- a3/a4: every query against the tile -----------------------------------------------------------
             for (int32_t q = 0; q < nq; q++) {
                 const int32_t m = qlen[q];
-                if (m == 0) { if (lane == 0) wres[q * C::NW + warp] = 0u; continue; }
+                if (m == 0 || ((skipq >> q) & 1u)) { if (lane == 0) wres[q * C::NW + warp] = 0u; continue; }
                 const int32_t need = thr[q >> (ns - 1)];       // the read's current second-best score (or -1)
                 const uint32_t* ro = roff + q * MP;
                 uint32_t H[K], B[K];

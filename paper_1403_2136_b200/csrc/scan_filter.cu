@@ -166,7 +166,7 @@ scan_filter_kernel(ScanParams p, FilterGeom ug, int32_t MP, int32_t ROWW, uint16
 }
 
 struct FVariant { int K, T; };
-const FVariant kFVariants[] = { {4, 256}, {4, 128}, {4, 64} };
+const FVariant kFVariants[] = { {4, 256}, {4, 128}, {4, 64}, {8, 128}, {8, 256} };
 
 struct FSmem { int32_t MP, ROWW; size_t bytes; };
 FSmem filter_smem(int half, int nw, int32_t max_len, int32_t istep)
@@ -182,8 +182,14 @@ FSmem filter_smem(int half, int nw, int32_t max_len, int32_t istep)
 }
 
 // the tile with the least padding among those that leave room for two blocks per SM; -1 = none
+int g_filter_force = -1;      // tuning hook (mss_set_scan_variant 8..12): force one pass-1 tile geometry
+
 int pick_filter_variant(const mss_genome* g, const ScanParams& p)
 {
+    if (g_filter_force >= 0 && g_filter_force < 5) {
+        const FVariant& v = kFVariants[g_filter_force];
+        if (filter_smem(v.K * v.T, v.T / 32, p.max_len, p.istep).bytes + 2048 <= (size_t)g->max_smem_optin) return g_filter_force;
+    }
     int best = -1; double best_waste = 1e30;
     for (int i = 0; i < 3; i++) {
         const FVariant& v = kFVariants[i];
@@ -228,6 +234,8 @@ cudaError_t launch_filter_variant(const mss_genome* g, const ScanParams& p, uint
 
 }  // namespace
 
+void scan_filter_force_variant(int v) { g_filter_force = v; }
+
 bool scan_filter_supported(const mss_genome* g, const ScanParams& p)
 {
     if (p.pssm) return false;                                   // position-specific scores: one-pass scan only
@@ -251,6 +259,8 @@ cudaError_t launch_scan_filter(const mss_genome* g, const ScanParams& p, uint16_
     switch (v) {
         case 0: return launch_filter_variant<4, 256>(g, p, ubound, st, grid_out, smem_out);
         case 1: return launch_filter_variant<4, 128>(g, p, ubound, st, grid_out, smem_out);
-        default: return launch_filter_variant<4, 64>(g, p, ubound, st, grid_out, smem_out);
+        case 2: return launch_filter_variant<4, 64>(g, p, ubound, st, grid_out, smem_out);
+        case 3: return launch_filter_variant<8, 128>(g, p, ubound, st, grid_out, smem_out);
+        default: return launch_filter_variant<8, 256>(g, p, ubound, st, grid_out, smem_out);
     }
 }
