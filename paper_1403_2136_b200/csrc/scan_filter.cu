@@ -120,7 +120,8 @@ scan_filter_kernel(ScanParams p, FilterGeom ug, int32_t MP, int32_t ROWW, uint16
                 uint32_t H[K], B[K];
 #pragma unroll
                 for (int k = 0; k < K; k++) { H[k] = 0u; B[k] = 0u; }
-                for (int32_t j0 = 0; j0 < m2; j0 += 4) {
+                int32_t j0 = 0;
+                for (; j0 + 4 <= m2; j0 += 4) {
                     const uint4 o = *reinterpret_cast<const uint4*>(ro + j0);
                     uint32_t Ha[K];
 #pragma unroll
@@ -135,6 +136,24 @@ scan_filter_kernel(ScanParams p, FilterGeom ug, int32_t MP, int32_t ROWW, uint16
                     for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.w + k * T * 4), zero);
 #pragma unroll
                     for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                }
+                if (m2 & 2) {                                   // remainder: two double steps ...
+                    const uint2 o = *reinterpret_cast<const uint2*>(ro + j0);
+                    uint32_t Ha[K];
+#pragma unroll
+                    for (int k = 0; k < K; k++) Ha[k] = __viaddmax_s16x2(H[k], *reinterpret_cast<const uint32_t*>(my + o.x + k * T * 4), zero);
+#pragma unroll
+                    for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(Ha[k], *reinterpret_cast<const uint32_t*>(my + o.y + k * T * 4), zero);
+#pragma unroll
+                    for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                    j0 += 2;
+                }
+                if (m2 & 1) {                                   // ... and / or one
+                    const uint32_t o = ro[j0];
+#pragma unroll
+                    for (int k = 0; k < K; k++) H[k] = __viaddmax_s16x2(H[k], *reinterpret_cast<const uint32_t*>(my + o + k * T * 4), zero);
+#pragma unroll
+                    for (int k = 0; k < K; k++) B[k] = __vmaxs2(B[k], H[k]);
                 }
                 if (nvalid < D) {                               // ragged last tile: drop foreign window starts
 #pragma unroll
