@@ -83,3 +83,34 @@ def test_cells_formula():
     cfg = gen.config(2)
     assert cfg.cells() == 100_000 * 100 * 1124 * 4096 * 2
     assert gen.config(1).cells() == 200 * 100 * 50 * 1000
+
+
+def test_quals_are_seeded_and_in_range():
+    """gen.make_quals: same seed -> same bytes; phred values in [2, 41]; a share of reads carries a Q2 tail."""
+    a = gen.make_quals(500, 100, 123)
+    b = gen.make_quals(500, 100, 123)
+    c = gen.make_quals(500, 100, 124)
+    assert a.dtype == np.uint8 and a.shape == (500, 100)
+    assert (a == b).all() and (a != c).any()
+    assert a.min() >= 2 and a.max() <= 41
+    tails = (a[:, -1] == 2).mean()
+    assert 0.05 < tails < 0.3
+
+
+def test_chunked_packing_equals_one_shot(monkeypatch):
+    """pack_2bit works chunk by chunk for Gbp-sized genomes: any chunk size gives the same words."""
+    from gen import synth
+    rng = np.random.default_rng(9)
+    codes = rng.integers(0, 5, size=200_003).astype(np.uint8)
+    whole = gen.pack_2bit(codes)
+    monkeypatch.setattr(synth, "_PACK_CHUNK", 4096)
+    parts = gen.pack_2bit(codes)
+    assert (whole[0] == parts[0]).all() and (whole[1] == parts[1]).all()
+    assert (gen.unpack_2bit(parts[0], parts[1], codes.size) == codes).all()
+
+
+def test_config6_is_the_table8_shape():
+    """PAPER.md:182, Table 8: 76 bp reads against a 2.4 Gbp genome, fragment length 4800."""
+    cfg = gen.config(6)
+    assert (cfg.genome_len, cfg.frag_len, cfg.max_len, cfg.strands) == (2_400_000_000, 4800, 76, 3)
+    assert -(-cfg.genome_len // cfg.frag_len) == 500_000
