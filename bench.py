@@ -28,7 +28,7 @@ import gen  # noqa: E402
 
 ALGO_INSTR_PER_CELL = 0.75          # one-pass scan: 1 VIADDMNMX.S16x2 per 2 cells + 1 VIMNMX3.S16x2 per 4 cells
 ALGO_INSTR_PER_CELL_PASS1 = 0.375   # two-pass scan, pass 1: 1 VIADDMNMX.S16x2 per 4 cells + 1 VIMNMX3.S16x2 per 8 cells
-NCU_DRAM_BYTES_PASS1 = 2_048_000     # profiles/r1_scan_filter_full.md (2.03 MB read + 0.02 MB written per launch)
+NCU_DRAM_BYTES_PASS1 = 2_019_072     # profiles/r1_scan_filter_full.md (2.00 MB read + 0.02 MB written per launch)
 NCU_DRAM_BYTES_PER_LAUNCH = 2_043_648   # profiles/r1_scan_dpx_full.md (2.04 MB read + 0 written per launch)
 ALU_LANES_PER_CLK_SM = 64           # integer/DPX pipe: 16 lanes/clk per SM sub-partition x 4 (guide + measured)
 
