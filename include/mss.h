@@ -248,6 +248,9 @@ int mss_get_last_launch(mss_launch_info_t *out);
  * of the latest such call and returns the summed milliseconds (0, 0 if that call took another path).
  */
 int mss_set_pass_timing(int on);
+/* Bytes of pass-1 bounds produced per chunk of reads (default 1 GiB, <= 0 restores it; process-wide).  The workspace
+ * queries follow it.  Results do not depend on it; tests set it small to exercise the chunk loop. */
+int mss_set_two_pass_chunk_bytes(int64_t bytes);
 int mss_get_pass_times(float *h_pass1_ms, float *h_pass2_ms);
 
 /*

@@ -80,6 +80,7 @@ def lib() -> C.CDLL:
     L.mss_nw_align.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, _Scoring, i32, vp, sz, vp, vp, vp, vp, i32, vp]
     L.mss_nw_align.restype = C.c_int
     L.mss_mapq_filter.argtypes = [vp, i32, C.c_float, vp, vp, vp]; L.mss_mapq_filter.restype = C.c_int
+    L.mss_set_two_pass_chunk_bytes.argtypes = [C.c_int64]; L.mss_set_two_pass_chunk_bytes.restype = C.c_int
     L.mss_set_pass_timing.argtypes = [C.c_int]; L.mss_set_pass_timing.restype = C.c_int
     L.mss_get_pass_times.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]; L.mss_get_pass_times.restype = C.c_int
     L.mss_map_reads_bounds.argtypes = [vp, vp, vp, i32, vp, i32, i32, _Scoring, i32, i32, vp, vp, C.POINTER(i32)]
@@ -362,6 +363,10 @@ def mss_mapq_filter(d_hits, mapq_threshold: float = 15.2, stream=None):
     _check(lib().mss_mapq_filter(_ptr(d_hits), n, float(mapq_threshold), _stream(stream), _ptr(mapped), _ptr(mapq)),
            "mss_mapq_filter")
     return mapped, mapq
+
+
+def mss_set_two_pass_chunk_bytes(nbytes: int) -> None:
+    _check(lib().mss_set_two_pass_chunk_bytes(int(nbytes)), "mss_set_two_pass_chunk_bytes")
 
 
 def mss_set_pass_timing(on: bool) -> None:

@@ -374,6 +374,8 @@ int mss_set_scan_variant(int variant)
     return MSS_OK;
 }
 
+int mss_set_two_pass_chunk_bytes(int64_t bytes) { scan_set_two_pass_chunk_bytes(bytes); return MSS_OK; }
+
 int mss_set_pass_timing(int on) { scan_set_pass_timing(on != 0); return MSS_OK; }
 
 int mss_get_pass_times(float* h_pass1_ms, float* h_pass2_ms)

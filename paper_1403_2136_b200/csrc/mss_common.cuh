@@ -121,6 +121,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p, void*
                                  mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info);
 
 void scan_set_pass_timing(bool on);
+void scan_set_two_pass_chunk_bytes(int64_t bytes);
 cudaError_t scan_get_pass_times(float* pass1_ms, float* pass2_ms);
 
 size_t nw_workspace(const mss_genome* g, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t pad);

@@ -463,10 +463,12 @@ cudaEvent_t next_event()
     return (*t_events)[t_events_used++];
 }
 
+int64_t g_bounds_bytes = 1ll << 30;   // bounds produced per chunk of reads (mss_set_two_pass_chunk_bytes: tests use small values)
+
 int32_t two_pass_chunk(const mss_genome* g, int32_t n_reads, int32_t strands)
 {
     int64_t per_read = (int64_t)(strands == 3 ? 2 : 1) * g->n_frag * 2;         // bytes of bounds per read
-    int64_t c = (1ll << 30) / per_read;
+    int64_t c = g_bounds_bytes / per_read;
     if (c < 1) c = 1;
     if (c > n_reads) c = n_reads;
     if (c < 1) c = 1;
@@ -525,6 +527,8 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
     }
     return cudaSuccess;
 }
+
+void scan_set_two_pass_chunk_bytes(int64_t bytes) { g_bounds_bytes = bytes < 1 ? (1ll << 30) : bytes; }
 
 void scan_set_pass_timing(bool on) { t_time_passes = on; if (!on) t_events_used = 0; }
 

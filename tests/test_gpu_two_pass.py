@@ -134,3 +134,25 @@ def test_two_pass_other_scorings_and_long_reads(oracle_mod):
     G = load_genome(g, 2048, -1)
     want = oracle_mod.map_reads_parallel(g, 2048, -1, r["reads"], r["lens"], strands=3)
     _cmp(map_reads(G, r["reads"], r["lens"], variant=7), want, "m=700")
+
+
+def test_two_pass_chunk_loop(oracle_mod):
+    """The bounds are produced per chunk of reads (1 GiB by default).  With a 20 kB limit the 200 reads of the tiny config
+    take dozens of chunks (ragged last chunk included); the records must not change."""
+    import paper_1403_2136_b200 as mss
+    from gpu_util import load_genome, map_reads
+    cfg = gen.config(1)
+    g, _ = cfg.genome()
+    r = cfg.reads(g)
+    reads, lens = r["reads"].copy(), r["lens"]
+    reads[1::2] = np.stack([gen.revcomp(x) for x in reads[1::2]])
+    want = oracle_mod.map_reads_parallel(g, cfg.frag_len, -1, reads, lens, strands=3)
+    G = load_genome(g, cfg.frag_len, -1)
+    try:
+        for nbytes in (20_000, 1400, 200):                # 100, 7 and 1 reads per chunk (50 fragments x 2 strands x 2 B per read)
+            mss.mss_set_two_pass_chunk_bytes(nbytes)
+            got = map_reads(G, reads, lens, strands=3, variant=7)
+            assert mss.mss_get_last_launch()["launches"] >= 2 * (200 * 200 // nbytes)
+            _cmp(got, want, f"chunk bytes {nbytes}")
+    finally:
+        mss.mss_set_two_pass_chunk_bytes(0)
