@@ -33,6 +33,7 @@ def main():
     ap.add_argument("--mode", default="plain", choices=["plain", "fast", "pssm"])
     ap.add_argument("--nw-reads", type=int, default=4096, help="reads whose second stage is also compared (evenly spaced)")
     ap.add_argument("--skip", type=int, default=0, help="compare only reads [skip, n) with the oracle (the GPU still maps all)")
+    ap.add_argument("--stop", type=int, default=None, help="compare only reads [skip, stop) (one gpurun call lasts at most an hour)")
     ap.add_argument("--variant", type=int, default=0, help="scan variant (0 = automatic, 7 = two-pass)")
     ap.add_argument("--chunk", type=int, default=2048)
     ap.add_argument("--workers", type=int, default=None,
@@ -83,8 +84,9 @@ def main():
     bad_top2, checked = [], 0
     t0 = time.perf_counter()
     want_all = np.zeros_like(got)
-    for a in range(args.skip, n, args.chunk):
-        b = min(n, a + args.chunk)
+    stop = n if args.stop is None else min(n, args.stop)
+    for a in range(args.skip, stop, args.chunk):
+        b = min(stop, a + args.chunk)
         if args.mode == "pssm":
             want = oracle.map_reads_pssm_parallel(genome, cfg.frag_len, cfg.overlap, reads[a:b], lens[a:b], pm[a:b], pmm[a:b],
                                                   strands=cfg.strands, workers=cores)
@@ -100,7 +102,7 @@ def main():
     cpu_s = time.perf_counter() - t0
 
     # second stage on an evenly spaced subset (the oracle's full-matrix NW is the slow part there)
-    idx = np.unique(np.linspace(args.skip, n - 1, min(n - args.skip, args.nw_reads)).astype(np.int64))
+    idx = np.unique(np.linspace(args.skip, stop - 1, min(stop - args.skip, args.nw_reads)).astype(np.int64))
     if args.mode == "pssm":
         ws, wp, wc, wn = oracle.nw_align_pssm(genome, cfg.frag_len, cfg.overlap, reads[idx], lens[idx], want_all[idx], pm[idx],
                                               pmm[idx], scale * sc.gap, cigar_stride=64)
