@@ -158,6 +158,9 @@ def main():
 
     import torch
     import paper_1403_2136_b200 as mss
+    if not os.path.exists(mss.lib_path()) and int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        from paper_1403_2136_b200 import build as mss_build      # in-tree build of libmss.so (nvcc, sm_100a); no fallback exists
+        mss_build.build()
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

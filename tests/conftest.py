@@ -17,3 +17,14 @@ def oracle_mod():
     import oracle
     oracle.build()
     return oracle
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _libmss_present():
+    """libmss.so is built in-tree (python -m paper_1403_2136_b200.build / __graft_entry__.build()); if a checkout has none
+    yet and nvcc is at hand, build it once so that the ABI and GPU tests exercise the CUDA path (there is no fallback)."""
+    import shutil
+    from paper_1403_2136_b200 import binding, build as mss_build
+    if not os.path.exists(binding.lib_path()) and (shutil.which("nvcc") or os.path.exists("/usr/local/cuda/bin/nvcc")):
+        mss_build.build()
+    yield
