@@ -161,6 +161,10 @@ def main():
     if not os.path.exists(mss.lib_path()) and int(os.environ.get("LOCAL_RANK", "0")) == 0:
         from paper_1403_2136_b200 import build as mss_build      # in-tree build of libmss.so (nvcc, sm_100a); no fallback exists
         mss_build.build()
+    for _ in range(600):                                         # other local ranks wait for rank 0's build
+        if os.path.exists(mss.lib_path()):
+            break
+        time.sleep(0.5)
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
