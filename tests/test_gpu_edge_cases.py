@@ -167,7 +167,8 @@ def test_long_reads_several_groups_all_modes(oracle_mod):
     _cmp(map_reads(G, reads, lens), oracle_mod.map_reads_parallel(g, 4096, -1, reads, lens, strands=3), "plain m=1500")
     _cmp(map_reads_fast(G, reads, lens), oracle_mod.map_reads_parallel(g, 4096, -1, reads, lens, strands=3, fast=True), "fast m=1500")
     quals = gen.make_quals(n, m, 2101)
-    d_pssm, pm, pmm = pssm_tables(quals, lens, scale=4)
+    d_pssm, _, _ = pssm_tables(quals, lens, scale=4)
+    pm, pmm = oracle_mod.pssm_from_phred(quals, 5, -4, 4)                     # the oracle's own table
     _cmp(map_reads_pssm(G, reads, lens, d_pssm, scale=4),
          oracle_mod.map_reads_pssm_parallel(g, 4096, -1, reads, lens, pm, pmm, strands=3), "pssm m=1500")
 

@@ -103,7 +103,9 @@ def test_pssm_geometries(oracle_mod, tiny, F, V, strands):
     from gpu_util import load_genome, map_reads_pssm, pssm_tables
     cfg, g, reads, lens, quals = tiny
     d_pssm, pm, pmm = pssm_tables(quals[:40], lens[:40])
-    want = oracle_mod.map_reads_pssm_parallel(g, F, V, reads[:40], lens[:40], pm, pmm, strands=strands)
+    wpm, wpmm = oracle_mod.pssm_from_phred(quals[:40], 5, -4, 16)            # the oracle's own table feeds the oracle
+    assert (pm == wpm).all() and (pmm == wpmm).all()
+    want = oracle_mod.map_reads_pssm_parallel(g, F, V, reads[:40], lens[:40], wpm, wpmm, strands=strands)
     G = load_genome(g, F, V)
     got = map_reads_pssm(G, reads[:40], lens[:40], d_pssm, strands=strands)
     _cmp(got, want, f"pssm F={F} V={V} strands={strands}")
@@ -125,7 +127,10 @@ def test_pssm_ragged_lengths_and_long_reads(oracle_mod, tiny):
         reads[i, :lens[i]] = gen.revcomp(rd) if i % 2 else rd
     quals = gen.make_quals(n, M, 77)
     d_pssm, pm, pmm = pssm_tables(quals, lens, scale=8)
-    want = oracle_mod.map_reads_pssm_parallel(g, 2048, -1, reads, lens, pm, pmm, strands=3)
+    wpm, wpmm = oracle_mod.pssm_from_phred(quals, 5, -4, 8)
+    valid = np.arange(M)[None, :] < lens[:, None]
+    assert (pm[valid] == wpm[valid]).all() and (pmm[valid] == wpmm[valid]).all() and (pm[~valid] == 0).all()
+    want = oracle_mod.map_reads_pssm_parallel(g, 2048, -1, reads, lens, wpm, wpmm, strands=3)
     G = load_genome(g, 2048, -1)
     _cmp(map_reads_pssm(G, reads, lens, d_pssm, strands=3, scale=8), want, "pssm ragged")
 
@@ -147,9 +152,11 @@ def test_pssm_uniform_table_equals_plain_scan(tiny):
 def test_nw_pssm_parity(oracle_mod, tiny):
     from gpu_util import load_genome, map_reads_pssm, nw_align_pssm, pssm_tables
     cfg, g, reads, lens, quals = tiny
-    d_pssm, pm, pmm = pssm_tables(quals, lens)
+    d_pssm, _, _ = pssm_tables(quals, lens)
+    pm, pmm = oracle_mod.pssm_from_phred(quals, 5, -4, 16)                    # oracle inputs come from the oracle only
     G = load_genome(g, cfg.frag_len, -1)
-    top2 = map_reads_pssm(G, reads, lens, d_pssm, strands=3)
+    top2 = oracle_mod.map_reads_pssm_parallel(g, cfg.frag_len, -1, reads, lens, pm, pmm, strands=3)
+    assert (map_reads_pssm(G, reads, lens, d_pssm, strands=3) == top2).all()
     want = oracle_mod.nw_align_pssm(g, cfg.frag_len, -1, reads, lens, top2, pm, pmm, 16 * -26)
     got = nw_align_pssm(G, reads, lens, top2, d_pssm)
     assert (got[0] == want[0]).all(), "score"
