@@ -12,14 +12,15 @@
 // (s1, s2) = (X, M) with H < -X), and an unsampled odd step lies at most -X above the next even one, hence
 //     Bt <= best <= Bt + delta,   delta = min(M, -X) - X.
 // The operand a depends on the read's base pair (c1, c2) and the genome pair (G[x], G[x+istep]): 16 "dibase" planes per
-// tile, plus 4 planes (c1, pad) with a = s1 for the last step of an odd-length query and one all-zero plane for dead
-// steps.  Queries holding an N (rare) are not scanned: their bound is 0xFFFF = "every fragment is a candidate".
+// tile, plus 4 planes (c1, pad) with a = s1 for the last step of an odd-length query (the loop runs the exact number of
+// double steps, so no padding steps exist).  Queries holding an N (rare) are not scanned: their bound is 0xFFFF =
+// "every fragment is a candidate".
 #include "mss_common.cuh"
 
 namespace {
 
 constexpr int FQ_MAX = 32;          // queries (read x strand) per block
-constexpr int NPLANE = 21;          // 4 x (4 + pad) dibase planes + the zero plane
+constexpr int NPLANE = 20;          // 4 x (4 + pad) dibase planes
 
 struct FilterGeom { int32_t n_groups, n_splits, frags_per_split, reads_per_group; };
 
@@ -62,7 +63,7 @@ scan_filter_kernel(ScanParams p, FilterGeom ug, int32_t MP, int32_t ROWW, uint16
         bool has_n = false;
         for (int32_t j = lane; j < MP; j += 32) {
             const int32_t i1 = 2 * j * istep, i2 = i1 + istep;  // the two read positions of double step j
-            uint32_t plane = 20u, col = (uint32_t)j;            // dead double step: the zero plane
+            uint32_t plane = 0u, col = 0u;                      // past the query's last double step: never read
             if (ok && i1 < m) {
                 uint32_t b1 = read_base(rw, rn, m, i1, strand);
                 uint32_t b2 = (i2 < m) ? read_base(rw, rn, m, i2, strand) : 5u;     // 5 = past the end (pad)
@@ -108,7 +109,6 @@ scan_filter_kernel(ScanParams p, FilterGeom ug, int32_t MP, int32_t ROWW, uint16
                         planes[(c1 * 5 + c2) * ROWW + x] = fpack2(sl + (lo2 == c2 ? M : X), sh + (hi2 == c2 ? M : X));
                     planes[(c1 * 5 + 4) * ROWW + x] = fpack2(sl, sh);
                 }
-                planes[20 * ROWW + x] = 0u;
             }
             __syncthreads();
 
