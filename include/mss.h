@@ -233,9 +233,10 @@ int mss_version(void);                         /* 100*major + minor */
 /*
  * Tuning / introspection (does not change results): select the scan kernel variant (0 = automatic: the two-pass scan
  * where the geometry allows it, else the one-pass tile kernel, else the generic kernel; 1 = generic; 2-6 = one-pass tile
- * kernels (K, T) = (8,256), (8,128), (8,64), (4,256), (16,128); 7 = two-pass, same as automatic) and report the
- * launch geometry of the last mss_map_reads call on this thread.  Used by bench.py and the parity tests to cover
- * every variant.
+ * kernels (K, T) = (8,256), (8,128), (8,64), (4,256), (16,128); 7 = two-pass, same as automatic; 8-12 = two-pass with
+ * the pass-1 tile (K, T) = (4,256), (4,128), (4,64), (8,128), (8,256) forced, process-wide, for tuning) and report the
+ * launch geometry of the last mss_map_reads call on this thread (two-pass: variant 7, grid / smem_bytes / tile_diagonals of
+ * pass 1, block 0, launches = 2 per chunk of reads).  Used by bench.py and the parity tests to cover every variant.
  */
 int mss_set_scan_variant(int variant);
 typedef struct { int32_t variant, grid, block, smem_bytes, reads_per_block, tile_diagonals, launches; } mss_launch_info_t;
