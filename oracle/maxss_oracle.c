@@ -15,7 +15,10 @@
  * enumeration of all fitting alignments for NW, planted-indel CIGARs.  The next-row functions at the end of the file
  * (MaxSSmap_fast, base-quality position-specific scoring) are pinned in tests/test_oracle_next_pins.py: brute force
  * over every scored sub-range, the decimated-sequence reduction to the pinned plain scan, the uniform-score reduction
- * to the pinned plain functions, closed-form phred values, exhaustive NW enumeration.  Nothing here is "parity unpinned".
+ * to the pinned plain functions, closed-form phred values, exhaustive NW enumeration.  oracle_mapq_filter (repeat filter +
+ * MAPQ) is pinned in tests/test_oracle_mapq_pins.py: the paper's printed pairs (.9 <-> 15.2, threshold 62), exact rational
+ * comparison for the .9 rule, closed forms at ratios 2^-k, the inverse relation through exact integer powers, edge readings.
+ * Nothing here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -444,5 +447,36 @@ void oracle_nw_align_pssm(const uint8_t *genome, int64_t G, int32_t F, int32_t V
         }
         ncig_out[r] = nc;
         free(ops); free(D); free(q); free(qm); free(qmm);
+    }
+}
+
+/*
+ * Repeat filter and mapping quality on the top-2 records of the first phase (next row f1).
+ *   PAPER.md:57 (section 2.2.1): "it outputs the fragment number with the highest and second highest score and considers
+ *   the read to be mapped if the ratio of the second best to best score is below .9".
+ *   "In the MAPQ field of SAM we use the formula -100 log2 p where p is the probability of alignment being
+ *   incorrect.  We define this to be the ratio of the scores of the second highest and top scoring fragments.  For
+ *   MaxSSmap we consider the read mapped only if mapping quality is above -100 log2 .9 = 15.2."
+ *   "we raise the MaxSSmap mapping quality threshold from the default 15.2 to 62".
+ * Per record, in this order:
+ *   - no best fragment (frag < 0) or best.score <= 0: the ratio is undefined -> unmapped, MAPQ 0 (reading 17);
+ *   - p = second.score / best.score in double, with second.score taken as 0 when there is no second fragment (a genome
+ *     of one fragment); p = 0 gives MAPQ = +infinity (nothing competes), otherwise MAPQ = -100 * log2(p) in double;
+ *   - threshold < 0 selects the paper's default in its exact form, "ratio below .9", decided on the integers
+ *     (10 * second < 9 * best) because the printed 15.2 is a rounded -100 log2 .9 = 15.2003 and would let a ratio of exactly .9
+ *     pass; threshold >= 0 is a mapping-quality cutoff as in PAPER.md:184: mapped iff MAPQ > threshold.
+ */
+void oracle_mapq_filter(const void *top2_v, int32_t n_reads, double threshold, uint8_t *mapped, double *mapq)
+{
+    const ohit_t *top2 = (const ohit_t *)top2_v;
+    for (int32_t r = 0; r < n_reads; r++) {
+        ohit_t best = top2[2 * r], second = top2[2 * r + 1];
+        if (best.frag < 0 || best.score <= 0) { mapped[r] = 0; mapq[r] = 0.0; continue; }
+        int32_t s2 = (second.frag >= 0) ? second.score : 0;
+        double p = (double)s2 / (double)best.score;
+        double q = (p > 0.0) ? -100.0 * log2(p) : INFINITY;
+        mapq[r] = q;
+        if (threshold < 0.0) mapped[r] = (10ll * (long long)s2 < 9ll * (long long)best.score) ? 1 : 0;
+        else mapped[r] = (q > threshold) ? 1 : 0;
     }
 }

@@ -60,6 +60,8 @@ def _lib(opt: str = "O2") -> C.CDLL:
         lib.oracle_nw_align_pssm.argtypes = [u8p, C.c_int64, C.c_int32, C.c_int32, u8p, C.c_int32, i32p, C.c_int32, vp,
                                              i32p, i32p, C.c_int32, C.c_int32, i32p, i64p, u32p, C.c_int32, i32p]
         lib.oracle_nw_align_pssm.restype = None
+        lib.oracle_mapq_filter.argtypes = [vp, C.c_int32, C.c_double, u8p, C.POINTER(C.c_double)]
+        lib.oracle_mapq_filter.restype = None
         _LIBS[opt] = lib
     return _LIBS[opt]
 
@@ -211,3 +213,15 @@ def nw_align_pssm(genome, frag_len, overlap, reads, lens, top2, pmatch, pmismatc
                                    _p(pm, C.c_int32), _p(pmm, C.c_int32), gap, pad, _p(score, C.c_int32),
                                    _p(pos, C.c_int64), _p(cig, C.c_uint32), stride, _p(ncig, C.c_int32))
     return score, pos, cig, ncig
+
+
+def mapq_filter(top2, threshold=-1.0, opt="O2"):
+    """Repeat filter + MAPQ on top-2 records -> (mapped uint8[n], mapq float64[n]).
+    threshold < 0: the paper's default "ratio below .9" decided on integers; >= 0: mapped iff MAPQ > threshold."""
+    top2 = np.ascontiguousarray(top2, dtype=np.int32).reshape(-1, 2, 4)
+    n = top2.shape[0]
+    mapped = np.zeros(n, dtype=np.uint8)
+    mapq = np.zeros(n, dtype=np.float64)
+    _lib(opt).oracle_mapq_filter(top2.ctypes.data_as(C.c_void_p), n, float(threshold), _p(mapped, C.c_uint8),
+                                 _p(mapq, C.c_double))
+    return mapped, mapq
