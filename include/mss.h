@@ -137,12 +137,17 @@ int mss_nw_align(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t 
 /* ---- repeat filter and mapping quality ------------------------------------------------ */
 
 /*
- * d_mapped[r] = 1 iff best.frag >= 0, best.score > 0 and MAPQ > mapq_threshold, where the ratio p = second/best
- * (second.frag < 0 or second.score = 0 -> p = 0, MAPQ = +inf reported as 3.4e38) and MAPQ = -100 log2 p (float32).
- * The paper's default threshold is -100 log2 0.9 = 15.2; the integer form 10*second < 9*best decides at exactly 15.2
- * (pass mapq_threshold < 0 to use that exact integer rule).  d_mapq may be NULL.
+ * Per record ("considers the read to be mapped if the ratio of the second best to best score is below .9";
+ * PAPER.md:63 MAPQ = -100 log2 p, p = second/best; PAPER.md:184 a stricter cutoff of 62):
+ *   - best.frag < 0 or best.score <= 0: the ratio is undefined -> d_mapped[r] = 0, d_mapq[r] = 0 (reading 17);
+ *   - p = second.score / best.score, second.score counting as 0 when second.frag < 0 (a genome of one fragment);
+ *     p = 0 -> MAPQ = +infinity, else MAPQ = -100 log2 p, computed in IEEE double and stored as float32;
+ *   - mapq_threshold < 0 (the default of the binding): the paper's rule in its exact form, mapped iff
+ *     10*second < 9*best on the integers (the printed 15.2 is a rounded -100 log2 .9 = 15.2003 and would admit a ratio of
+ *     exactly .9); mapq_threshold >= 0: mapped iff MAPQ > mapq_threshold, decided in double before the float32 store.
+ * d_mapq may be NULL.
  */
-int mss_mapq_filter(const mss_top2_t *d_hits, int32_t n_reads, float mapq_threshold,
+int mss_mapq_filter(const mss_top2_t *d_hits, int32_t n_reads, double mapq_threshold,
                     void *stream, uint8_t *d_mapped, float *d_mapq);
 
 /* ---- next rows: MaxSSmap_fast and base-quality position-specific scoring ------------------------------------------- */
@@ -234,9 +239,11 @@ int mss_version(void);                         /* 100*major + minor */
  * Tuning / introspection (does not change results): select the scan kernel variant (0 = automatic: the two-pass scan
  * where the geometry allows it, else the one-pass tile kernel, else the generic kernel; 1 = generic; 2-6 = one-pass tile
  * kernels (K, T) = (8,256), (8,128), (8,64), (4,256), (16,128); 7 = two-pass, same as automatic; 8-12 = two-pass with
- * the pass-1 tile (K, T) = (4,256), (4,128), (4,64), (8,128), (8,256) forced, process-wide, for tuning) and report the
+ * the pass-1 tile (K, T) = (4,256), (4,128), (4,64), (8,128), (8,256) forced; anything else: MSS_ERR_ARG) and report the
  * launch geometry of the last mss_map_reads call on this thread (two-pass: variant 7, grid / smem_bytes / tile_diagonals of
  * pass 1, block 0, launches = 2 per chunk of reads).  Used by bench.py and the parity tests to cover every variant.
+ * Every tuning switch of this section (scan variant, forced pass-1 tile, pass timing, bounds chunk size, queries per
+ * pass-1 block) is thread-local: it affects only calls made later on the same host thread.
  */
 int mss_set_scan_variant(int variant);
 typedef struct { int32_t variant, grid, block, smem_bytes, reads_per_block, tile_diagonals, launches; } mss_launch_info_t;
@@ -249,7 +256,7 @@ int mss_get_last_launch(mss_launch_info_t *out);
  * of the latest such call and returns the summed milliseconds (0, 0 if that call took another path).
  */
 int mss_set_pass_timing(int on);
-/* Bytes of pass-1 bounds produced per chunk of reads (default 1 GiB, <= 0 restores it; process-wide).  The workspace
+/* Bytes of pass-1 bounds produced per chunk of reads (default 256 MiB, <= 0 restores it; this thread only).  The workspace
  * queries follow it.  Results do not depend on it; tests set it small to exercise the chunk loop. */
 int mss_set_two_pass_chunk_bytes(int64_t bytes);
 int mss_get_pass_times(float *h_pass1_ms, float *h_pass2_ms);
@@ -276,17 +283,13 @@ int mss_map_reads_bounds(const mss_genome_t *g, const uint32_t *d_reads, const u
 int mss_probe_dpx_peak(int32_t iters, void *stream, double *h_instr_per_s, float *h_ms);
 
 /*
- * Issue-rate probes behind the roofline denominator: `which` selects an instruction or mix, the result
- * is thread-instructions (rows 11-13: cells) per clock per SM, measured with clock64 over `iters` rounds of 64 chain
- * steps on 1024 threads per SM.  0 VIADDMNMX.S16x2.RELU, 1 VIMNMX3.S16x2, 2 their 2:1 mix, 3 PRMT, 4 LOP3, 5 IMAD,
- * 6 HFMA2.RELU, 7 DPX+IMAD, 8 DPX+PRMT, 9 DPX+HFMA2.RELU (both counted), 10 LDS.32, 11 the scan's inner mix
- * (LDS.32 + VIADDMNMX per 2 cells + VIMNMX3 per 4 cells), 12 PRMT + HFMA2.RELU + VIMNMX3 mix, 13 PRMT + VIADDMNMX +
- * VIMNMX3 mix, 14 F2FP.F16.E4M3.UNPACK_B (fp8 pair -> f16x2), 15 DPX+F2FP, 16 HFMA2+F2FP (both counted), 17 byte-score mix
- * (LDS.32 per 4 cells + 2 F2FP + 2 HFMA2.RELU + VIMNMX3) [cells], 18 the same with PRMT as the widening [cells],
- * 19 hybrid of rows 11 and 17 on alternating chains [cells], 20 LDS.64, 21 LDS.128 (thread-loads; x8 / x16 bytes).
- * Synchronises the stream before returning.
+ * Issue-rate probes behind the roofline denominators: `which` selects an instruction or mix, the result
+ * is thread-instructions (row 4: cells) per clock per SM, measured with clock64 over `iters` rounds of 64 chain steps on
+ * 1024 threads per SM.  0 VIADDMNMX.S16x2.RELU, 1 VIMNMX3.S16x2, 2 their 2:1 mix, 3 LDS.32 conflict-free (x 4 B = the
+ * shared-memory feed), 4 the exact scan's inner mix (LDS.32 + VIADDMNMX per 2 cells + VIMNMX3 per 4 cells).
+ * Synchronises the stream before returning.  (The design-experiment rows of round 1 are no longer part of the library.)
  */
-enum { MSS_PROBE_COUNT = 22 };
+enum { MSS_PROBE_COUNT = 5 };
 int mss_probe_pipe(int32_t which, int32_t iters, void *stream, double *h_per_clk_sm);
 
 #ifdef __cplusplus

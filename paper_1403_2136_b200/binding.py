@@ -79,7 +79,7 @@ def lib() -> C.CDLL:
     L.mss_nw_workspace_bytes.argtypes = [vp, i32, i32, _Scoring, i32]; L.mss_nw_workspace_bytes.restype = sz
     L.mss_nw_align.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, _Scoring, i32, vp, sz, vp, vp, vp, vp, i32, vp]
     L.mss_nw_align.restype = C.c_int
-    L.mss_mapq_filter.argtypes = [vp, i32, C.c_float, vp, vp, vp]; L.mss_mapq_filter.restype = C.c_int
+    L.mss_mapq_filter.argtypes = [vp, i32, C.c_double, vp, vp, vp]; L.mss_mapq_filter.restype = C.c_int
     L.mss_set_two_pass_chunk_bytes.argtypes = [C.c_int64]; L.mss_set_two_pass_chunk_bytes.restype = C.c_int
     L.mss_set_pass_timing.argtypes = [C.c_int]; L.mss_set_pass_timing.restype = C.c_int
     L.mss_get_pass_times.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]; L.mss_get_pass_times.restype = C.c_int
@@ -354,8 +354,9 @@ def mss_nw_align(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, d_hits
     return score, pos, cigar, ncig
 
 
-def mss_mapq_filter(d_hits, mapq_threshold: float = 15.2, stream=None):
-    """-> (mapped uint8[n], mapq float32[n]); mapq_threshold < 0 selects the exact integer 0.9 rule."""
+def mss_mapq_filter(d_hits, mapq_threshold: float = -1.0, stream=None):
+    """-> (mapped uint8[n], mapq float32[n]); mapq_threshold < 0 (default) = the paper's "ratio below .9" on integers
+    (PAPER.md:57); >= 0 = mapped iff MAPQ > threshold."""
     torch = _torch()
     n = int(d_hits.shape[0])
     mapped = torch.empty(n, dtype=torch.uint8, device=d_hits.device)
@@ -397,16 +398,8 @@ def mss_probe_dpx_peak(iters: int = 4096, stream=None):
     return rate.value, ms.value
 
 
-PROBE_NAMES = ["VIADDMNMX.S16x2.RELU", "VIMNMX3.S16x2", "DPX mix 2:1 (relu : max3)", "PRMT", "LOP3", "IMAD", "HFMA2.RELU",
-               "DPX + IMAD 1:1 (both counted)", "DPX + PRMT 1:1 (both counted)", "DPX + HFMA2.RELU 1:1 (both counted)",
-               "LDS.32 (conflict-free)", "scan mix: LDS.32 + VIADDMNMX /2 cells + VIMNMX3 /4 cells  [cells]",
-               "alt mix: PRMT + HFMA2.RELU /2 cells + VIMNMX3 /4 cells  [cells]",
-               "alt mix: PRMT + VIADDMNMX /2 cells + VIMNMX3 /4 cells  [cells]",
-               "F2FP.F16.E4M3.UNPACK_B (fp8x2 -> f16x2)", "DPX + F2FP 1:1 (both counted)", "HFMA2.RELU + F2FP 1:1 (both counted)",
-               "byte mix: LDS.32 /4 cells + 2 F2FP + 2 HFMA2.RELU + VIMNMX3  [cells]",
-               "byte mix: LDS.32 /4 cells + 2 PRMT + 2 HFMA2.RELU + VIMNMX3  [cells]",
-               "hybrid: chains alternate scan mix (row 11) and byte mix (row 17)  [cells]",
-               "LDS.64 (conflict-free; x8 bytes)", "LDS.128 (conflict-free; x16 bytes)"]
+PROBE_NAMES = ["VIADDMNMX.S16x2.RELU", "VIMNMX3.S16x2", "DPX mix 2:1 (relu : max3)", "LDS.32 (conflict-free)",
+               "scan mix: LDS.32 + VIADDMNMX /2 cells + VIMNMX3 /4 cells  [cells]"]
 
 
 def mss_probe_pipe(which: int, iters: int = 2000, stream=None) -> float:

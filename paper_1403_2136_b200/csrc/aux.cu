@@ -1,26 +1,29 @@
 // Repeat filter / MAPQ on the top-2 records and the live DPX issue-rate probe.
+#include <math_constants.h>
 #include "mss_common.cuh"
 
-__global__ void mapq_kernel(const mss_top2_t* __restrict__ hits, int32_t n, float thr, uint8_t* __restrict__ mapped,
+// Decisions and the logarithm are taken in IEEE double (this file's --use_fast_math only touches single precision): the
+// default (thr < 0) is the paper's "ratio below .9" on the integers; a threshold >= 0 is a MAPQ cutoff.
+__global__ void mapq_kernel(const mss_top2_t* __restrict__ hits, int32_t n, double thr, uint8_t* __restrict__ mapped,
                             float* __restrict__ mapq)
 {
     int32_t r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
     mss_top2_t t = hits[r];
-    float q = 0.0f;
+    double q = 0.0;
     uint8_t ok = 0;
-    if (t.best.frag >= 0 && t.best.score > 0) {
+    if (t.best.frag >= 0 && t.best.score > 0) {                            // else: ratio undefined -> unmapped, MAPQ 0
         int32_t second = (t.second.frag >= 0) ? t.second.score : 0;
-        if (second <= 0) q = 3.4e38f;
-        else q = -100.0f * log2f((float)second / (float)t.best.score);
-        if (thr < 0.0f) ok = (10ll * second < 9ll * t.best.score) ? 1 : 0;   // the paper's 0.9 ratio, exact integers
+        if (second <= 0) q = CUDART_INF;                                    // p = 0: nothing competes
+        else q = -100.0 * log2((double)second / (double)t.best.score);
+        if (thr < 0.0) ok = (10ll * second < 9ll * t.best.score) ? 1 : 0;
         else ok = (q > thr) ? 1 : 0;
     }
     mapped[r] = ok;
-    if (mapq) mapq[r] = q;
+    if (mapq) mapq[r] = (float)q;
 }
 
-cudaError_t launch_mapq(const mss_top2_t* d_hits, int32_t n_reads, float thr, cudaStream_t st, uint8_t* d_mapped, float* d_mapq)
+cudaError_t launch_mapq(const mss_top2_t* d_hits, int32_t n_reads, double thr, cudaStream_t st, uint8_t* d_mapped, float* d_mapq)
 {
     mapq_kernel<<<(n_reads + 255) / 256, 256, 0, st>>>(d_hits, n_reads, thr, d_mapped, d_mapq);
     return cudaGetLastError();
@@ -96,26 +99,11 @@ cudaError_t run_dpx_probe(int32_t iters, cudaStream_t st, int sm_count, double* 
 }
 
 
-// ---- pipe issue-rate probes (evidence for the roofline denominator) ---------------------------------
-// Each probe runs 8 independent register chains per thread, 1024 threads x 1 block per SM, and reports
-// thread-instructions per clock per SM from clock64() around the loop.  Operands vary per thread so that nothing is
-// promoted to the uniform datapath.
+// ---- issue-rate probes behind the roofline denominators ---------------------------------------------
+// 8 independent register chains per thread, 1024 threads x 1 block per SM; thread-instructions (row 4: cells) per clock per
+// SM from clock64() around the loop.  Operands vary per thread so that nothing is promoted to the uniform datapath.
+// Rows: 0 VIADDMNMX.S16x2.RELU, 1 VIMNMX3.S16x2, 2 their 2:1 mix, 3 LDS.32 conflict-free, 4 the exact scan's inner mix.
 namespace {
-__device__ __forceinline__ uint32_t p_prmt(uint32_t a, uint32_t b, uint32_t s) { uint32_t d; asm volatile("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(s)); return d; }
-__device__ __forceinline__ uint32_t p_imad(uint32_t a, uint32_t b, uint32_t c) { uint32_t d; asm volatile("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c)); return d; }
-__device__ __forceinline__ uint32_t p_hfma2r(uint32_t a, uint32_t b, uint32_t c) { uint32_t d; asm volatile("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c)); return d; }
-__device__ __forceinline__ uint32_t p_lop3(uint32_t a, uint32_t b, uint32_t c) { uint32_t d; asm volatile("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(d) : "r"(a), "r"(b), "r"(c)); return d; }
-
-// fp8 e4m3 pair -> f16x2 (F2FP.F16.E4M3.UNPACK_B); HI selects the upper 16 bits of the source (operand .H1, no shift)
-template <bool HI>
-__device__ __forceinline__ uint32_t p_f2fp(uint32_t w)
-{
-    uint32_t d;
-    if (HI) asm volatile("{ .reg .b16 lo, hi; mov.b32 {lo, hi}, %1; cvt.rn.f16x2.e4m3x2 %0, hi; }" : "=r"(d) : "r"(w));
-    else    asm volatile("{ .reg .b16 lo, hi; mov.b32 {lo, hi}, %1; cvt.rn.f16x2.e4m3x2 %0, lo; }" : "=r"(d) : "r"(w));
-    return d;
-}
-
 template <int WHICH>
 __global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long long* cyc, uint32_t a, uint32_t b, uint32_t c, int iters)
 {
@@ -136,67 +124,13 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long lo
                 if (WHICH == 0) h[j] = __viaddmax_s16x2_relu(h[j], m[j], c);
                 if (WHICH == 1) h[j] = __vimax3_s16x2(h[j], m[j], c);
                 if (WHICH == 2) { h[j] = __viaddmax_s16x2_relu(h[j], m[j], c); if (j & 1) m[j] = __vimax3_s16x2(m[j], h[j], h[j - 1]); }
-                if (WHICH == 3) h[j] = p_prmt(h[j], m[j], c);
-                if (WHICH == 4) h[j] = p_lop3(h[j], m[j], c);
-                if (WHICH == 5) h[j] = p_imad(h[j], m[j], c);
-                if (WHICH == 6) h[j] = p_hfma2r(h[j], m[j], c);
-                if (WHICH == 7) { h[j] = __viaddmax_s16x2_relu(h[j], b, c); m[j] = p_imad(m[j], b, c); }
-                if (WHICH == 8) { h[j] = __viaddmax_s16x2_relu(h[j], b, c); m[j] = p_prmt(m[j], b, c); }
-                if (WHICH == 9) { h[j] = __viaddmax_s16x2_relu(h[j], b, c); m[j] = p_hfma2r(m[j], b, c); }
-                if (WHICH == 10) {   // LDS.32 only (conflict-free), one LOP3 consumer each
+                if (WHICH == 3) {   // LDS.32 only (conflict-free), one LOP3 consumer each
                     uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(myp + ((u * 8 + j) & 63) * 32 + (it & 1) * 2048)));
                     h[j] ^= v;
                 }
-                if (WHICH == 11) {   // the scan's inner mix: LDS.32 + VIADDMNMX.S16x2.RELU per 2 cells, VIMNMX3.S16x2 per 4 cells
+                if (WHICH == 4) {   // the exact scan's inner mix: LDS.32 + VIADDMNMX.S16x2.RELU per 2 cells, VIMNMX3.S16x2 per 4 cells
                     uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(myp + ((u * 8 + j) & 63) * 32 + (it & 1) * 2048)));
                     uint32_t hn = __viaddmax_s16x2_relu(h[j], v, c);
-                    if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
-                    h[j] = hn;
-                }
-                if (WHICH == 12) {   // alternative mix: PRMT table look-up + HFMA2.RELU per 2 cells, VIMNMX3.S16x2 per 4 cells
-                    uint32_t sc = p_prmt(m[j], b, h[(j + 1) & 7]);
-                    uint32_t hn = p_hfma2r(h[j], a, sc);
-                    if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
-                    h[j] = hn;
-                }
-                if (WHICH == 14) h[j] = p_f2fp<false>(h[j]) ^ 0u;
-                if (WHICH == 15) { h[j] = __viaddmax_s16x2_relu(h[j], b, c); m[j] = p_f2fp<true>(m[j]); }
-                if (WHICH == 16) { h[j] = p_hfma2r(h[j], b, c); m[j] = p_f2fp<true>(m[j]); }
-                if (WHICH == 17 || WHICH == 18) {
-                    // byte-score mixes: one LDS.32 carries 4 cells (fp8 / byte scores); per 4 cells 2 widenings
-                    // (17: F2FP e4m3x2->f16x2, 18: PRMT) + 2 HFMA2.RELU (Kadane in exact fp16) + 1 VIMNMX3.S16x2
-                    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(myp + ((u * 8 + j) & 63) * 32 + (it & 1) * 2048)));
-                    uint32_t s0 = WHICH == 17 ? p_f2fp<false>(v) : p_prmt(v, c, 0x1404u);
-                    uint32_t s1 = WHICH == 17 ? p_f2fp<true>(v) : p_prmt(v, c, 0x3424u);
-                    uint32_t h1 = p_hfma2r(h[j], a, s0);
-                    uint32_t h2 = p_hfma2r(h1, a, s1);
-                    m[j] = __vimax3_s16x2(m[j], h1, h2);
-                    h[j] = h2;
-                }
-                if (WHICH == 19) {   // hybrid: even chains as row 11 (LDS.32 + DPX per 2 cells), odd chains as row 17 at half rate
-                    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(myp + ((u * 8 + j) & 63) * 32 + (it & 1) * 2048)));
-                    if (j & 1) {
-                        uint32_t h1 = p_hfma2r(h[j], a, p_f2fp<false>(v));
-                        uint32_t h2 = p_hfma2r(h1, a, p_f2fp<true>(v));
-                        m[j] = __vimax3_s16x2(m[j], h1, h2);
-                        h[j] = h2;
-                    } else {
-                        uint32_t hn = __viaddmax_s16x2_relu(h[j], v, c);
-                        if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
-                        h[j] = hn;
-                    }
-                }
-                if (WHICH == 20) {   // LDS.64 (conflict-free): bytes per clock, not instructions, are what it shows
-                    uint32_t v0, v1; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v0), "=r"(v1) : "r"((uint32_t)__cvta_generic_to_shared(sm + 2 * threadIdx.x + ((u * 8 + j) & 1) * 2048 + ((h[j] >> 7) & 1) * 4096)));
-                    h[j] ^= v0; m[j] ^= v1;
-                }
-                if (WHICH == 21) {   // LDS.128 (conflict-free)
-                    uint32_t v0, v1, v2, v3; asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3) : "r"((uint32_t)__cvta_generic_to_shared(sm + 4 * threadIdx.x + ((h[j] >> 7) & 1) * 4096)));
-                    h[j] ^= v0 ^ v2; m[j] ^= v1 ^ v3;
-                }
-                if (WHICH == 13) {   // alternative mix, all on the ALU pipe: PRMT + VIADDMNMX per 2 cells, VIMNMX3 per 4 cells
-                    uint32_t sc = p_prmt(m[j], b, h[(j + 1) & 7]);
-                    uint32_t hn = __viaddmax_s16x2_relu(h[j], sc, c);
                     if (u & 1) m[j] = __vimax3_s16x2(m[j], h[j], hn);
                     h[j] = hn;
                 }
@@ -211,7 +145,7 @@ __global__ void __launch_bounds__(1024) pipe_probe_kernel(uint32_t* out, long lo
     if (threadIdx.x == 0) cyc[blockIdx.x] = t1 - t0;
 }
 
-const double kProbeCount[22] = { 1, 1, 1.5, 1, 1, 1, 1, 2, 2, 2, 1, 2, 2, 2, 1, 2, 2, 4, 4, 3, 1, 1 };   // counted units per chain step (mix rows 11-13: cells)
+const double kProbeCount[MSS_PROBE_COUNT] = { 1, 1, 1.5, 1, 2 };   // counted units per chain step (row 4: cells)
 
 template <int WHICH>
 cudaError_t launch_pipe_probe(uint32_t* out, long long* cyc, int blocks, int iters, cudaStream_t st)
@@ -223,7 +157,7 @@ cudaError_t launch_pipe_probe(uint32_t* out, long long* cyc, int blocks, int ite
 
 cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_count, double* per_clk_sm)
 {
-    if (which < 0 || which > 21) return cudaErrorInvalidValue;
+    if (which < 0 || which >= MSS_PROBE_COUNT) return cudaErrorInvalidValue;
     uint32_t* out = nullptr; long long* cyc = nullptr;
     int blocks = sm_count;
     cudaError_t e = cudaMalloc(&out, (size_t)blocks * 1024 * 4);                 // probe only: not on the mapping path
@@ -235,24 +169,7 @@ cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_cou
             case 1: e = launch_pipe_probe<1>(out, cyc, blocks, iters, st); break;
             case 2: e = launch_pipe_probe<2>(out, cyc, blocks, iters, st); break;
             case 3: e = launch_pipe_probe<3>(out, cyc, blocks, iters, st); break;
-            case 4: e = launch_pipe_probe<4>(out, cyc, blocks, iters, st); break;
-            case 5: e = launch_pipe_probe<5>(out, cyc, blocks, iters, st); break;
-            case 6: e = launch_pipe_probe<6>(out, cyc, blocks, iters, st); break;
-            case 7: e = launch_pipe_probe<7>(out, cyc, blocks, iters, st); break;
-            case 8: e = launch_pipe_probe<8>(out, cyc, blocks, iters, st); break;
-            case 9: e = launch_pipe_probe<9>(out, cyc, blocks, iters, st); break;
-            case 10: e = launch_pipe_probe<10>(out, cyc, blocks, iters, st); break;
-            case 11: e = launch_pipe_probe<11>(out, cyc, blocks, iters, st); break;
-            case 12: e = launch_pipe_probe<12>(out, cyc, blocks, iters, st); break;
-            case 13: e = launch_pipe_probe<13>(out, cyc, blocks, iters, st); break;
-            case 14: e = launch_pipe_probe<14>(out, cyc, blocks, iters, st); break;
-            case 15: e = launch_pipe_probe<15>(out, cyc, blocks, iters, st); break;
-            case 16: e = launch_pipe_probe<16>(out, cyc, blocks, iters, st); break;
-            case 17: e = launch_pipe_probe<17>(out, cyc, blocks, iters, st); break;
-            case 18: e = launch_pipe_probe<18>(out, cyc, blocks, iters, st); break;
-            case 19: e = launch_pipe_probe<19>(out, cyc, blocks, iters, st); break;
-            case 20: e = launch_pipe_probe<20>(out, cyc, blocks, iters, st); break;
-            default: e = launch_pipe_probe<21>(out, cyc, blocks, iters, st); break;
+            default: e = launch_pipe_probe<4>(out, cyc, blocks, iters, st); break;
         }
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);

@@ -17,6 +17,16 @@ int64_t padded_len(int64_t n_bases, int32_t frag_len)
     return (need + 127) / 128 * 128;
 }
 
+// the handle belongs to the device that was current at mss_genome_load: its pointers, SM count and shared-memory limit
+// mean nothing elsewhere, so a call made with another device current is refused instead of launched
+int check_device(const mss_genome* g)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return dev == g->device ? MSS_OK : MSS_ERR_ARG;
+}
+
 int check_scoring_scan(mss_scoring_t sc, int32_t max_len)
 {
     if (sc.match <= 0 || sc.mismatch >= 0) return MSS_ERR_RANGE;
@@ -97,6 +107,7 @@ static int map_reads_impl(const mss_genome_t* g, const uint32_t* d_reads, const 
     if ((int64_t)read_stride_words * 16 < max_len) return MSS_ERR_ARG;
     int rc = check_scoring_scan(sc, max_len);
     if (rc != MSS_OK) return rc;
+    if ((rc = check_device(g)) != MSS_OK) return rc;
     if (workspace_bytes < mss_map_workspace_bytes(g, n_reads, max_len, strands)) return MSS_ERR_WORKSPACE;
     ScanParams p;
     p.gpacked = g->packed; p.gnmask = g->nmask; p.n_bases = g->n_bases;
@@ -141,6 +152,7 @@ int mss_map_reads_bounds(const mss_genome_t* g, const uint32_t* d_reads, const u
     if ((int64_t)read_stride_words * 16 < max_len) return MSS_ERR_ARG;
     int rc = check_scoring_scan(sc, max_len);
     if (rc != MSS_OK) return rc;
+    if ((rc = check_device(g)) != MSS_OK) return rc;
     ScanParams p;
     p.gpacked = g->packed; p.gnmask = g->nmask; p.n_bases = g->n_bases;
     p.F = g->frag_len; p.V = g->overlap; p.n_frag = g->n_frag;
@@ -221,12 +233,14 @@ int mss_map_reads_host(const mss_genome_t* g, const uint32_t* h_reads, const uin
     cudaError_t e = cudaMemcpyAsync(d_reads, h_reads, reads_b, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess && h_reads_nmask) e = cudaMemcpyAsync(d_mask, h_reads_nmask, mask_b, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_lens, h_lens, lens_b, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return cuda_fail(e);
+    // from here on copies from / to the caller's host buffers may be in flight: no return without a synchronise
+    if (e != cudaSuccess) { cudaStreamSynchronize(st); return cuda_fail(e); }
     int rc = mss_map_reads(g, d_reads, h_reads_nmask ? d_mask : nullptr, read_stride_words, d_lens, n_reads, max_len, sc,
                            strands, d_workspace, base, st, d_out);
-    if (rc != MSS_OK) return rc;
+    if (rc != MSS_OK) { cudaStreamSynchronize(st); return rc; }
     e = cudaMemcpyAsync(h_out, d_out, n * sizeof(mss_top2_t), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaError_t es = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = es;
     if (e != cudaSuccess) return cuda_fail(e);
     return MSS_OK;
 }
@@ -251,6 +265,8 @@ static int nw_align_impl(const mss_genome_t* g, const uint32_t* d_reads, const u
     if (max_len > MSS_MAX_READ_LEN) return MSS_ERR_RANGE;
     if ((int64_t)max_len * (int64_t)(-sc.gap) > (1ll << 30) || (int64_t)max_len * sc.match > (1ll << 30)) return MSS_ERR_RANGE;
     if (workspace_bytes < mss_nw_workspace_bytes(g, n_reads, max_len, sc, pad)) return MSS_ERR_WORKSPACE;
+    int rcd = check_device(g);
+    if (rcd != MSS_OK) return rcd;
     cudaError_t e = launch_nw(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, d_hits, d_pssm, pssm_stride,
                               sc, pad, d_workspace, workspace_bytes, (cudaStream_t)stream, d_score, d_ref_pos, d_cigar,
                               cigar_stride, d_n_cigar);
@@ -322,24 +338,26 @@ int mss_map_align_host(const mss_genome_t* g, const uint32_t* h_reads, const uin
     cudaError_t e = cudaMemcpyAsync(d_reads, h_reads, reads_b, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess && h_reads_nmask) e = cudaMemcpyAsync(d_mask, h_reads_nmask, mask_b, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_lens, h_lens, n * 4, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return cuda_fail(e);
+    // from here on copies from / to the caller's host buffers may be in flight: no return without a synchronise
+    if (e != cudaSuccess) { cudaStreamSynchronize(st); return cuda_fail(e); }
     const uint32_t* dm = h_reads_nmask ? d_mask : nullptr;
     int rc = mss_map_reads(g, d_reads, dm, read_stride_words, d_lens, n_reads, max_len, sc, strands, d_workspace, scratch, st, d_top2);
-    if (rc != MSS_OK) return rc;
+    if (rc != MSS_OK) { cudaStreamSynchronize(st); return rc; }
     rc = mss_nw_align(g, d_reads, dm, read_stride_words, d_lens, n_reads, max_len, d_top2, sc, pad, d_workspace, scratch, st,
                       d_score, d_pos, d_cigar, cigar_stride, d_ncig);
-    if (rc != MSS_OK) return rc;
+    if (rc != MSS_OK) { cudaStreamSynchronize(st); return rc; }
     e = cudaMemcpyAsync(h_top2, d_top2, n * sizeof(mss_top2_t), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_score, d_score, n * 4, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_ref_pos, d_pos, n * 8, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_cigar, d_cigar, n * (size_t)cigar_stride * 4, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_n_cigar, d_ncig, n * 4, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaError_t es = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = es;
     if (e != cudaSuccess) return cuda_fail(e);
     return MSS_OK;
 }
 
-int mss_mapq_filter(const mss_top2_t* d_hits, int32_t n_reads, float mapq_threshold, void* stream, uint8_t* d_mapped, float* d_mapq)
+int mss_mapq_filter(const mss_top2_t* d_hits, int32_t n_reads, double mapq_threshold, void* stream, uint8_t* d_mapped, float* d_mapq)
 {
     if (n_reads < 0) return MSS_ERR_ARG;
     if (n_reads == 0) return MSS_OK;
@@ -366,7 +384,7 @@ int mss_version(void) { return 100; }
 
 int mss_set_scan_variant(int variant)
 {
-    if (variant < 0 || variant > 16) return MSS_ERR_ARG;
+    if (variant < 0 || variant > 12) return MSS_ERR_ARG;
     // 8..12: the two-pass scan with one pass-1 tile geometry forced (tuning); otherwise pass 1 picks its own
     scan_filter_force_variant(variant >= 8 && variant <= 12 ? variant - 8 : -1);
     if (variant >= 8 && variant <= 12) variant = 7;

@@ -134,6 +134,6 @@ cudaError_t launch_nw(const mss_genome* g, const uint32_t* d_reads, const uint32
 struct PssmLut { uint32_t v[94]; };   // phred 0..93 -> packed (pmatch, pmismatch), computed on the host in double
 cudaError_t launch_pssm_build(const uint8_t* d_qual, int32_t qual_stride, const int32_t* d_lens, int32_t n_reads,
                               const PssmLut& lut, cudaStream_t st, uint32_t* d_pssm, int32_t pssm_stride);
-cudaError_t launch_mapq(const mss_top2_t* d_hits, int32_t n_reads, float thr, cudaStream_t st, uint8_t* d_mapped, float* d_mapq);
+cudaError_t launch_mapq(const mss_top2_t* d_hits, int32_t n_reads, double thr, cudaStream_t st, uint8_t* d_mapped, float* d_mapq);
 cudaError_t run_dpx_probe(int32_t iters, cudaStream_t st, int sm_count, double* instr_per_s, float* ms);
 cudaError_t run_pipe_probe(int which, int32_t iters, cudaStream_t st, int sm_count, double* per_clk_sm);

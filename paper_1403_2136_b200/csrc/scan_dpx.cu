@@ -463,7 +463,7 @@ cudaEvent_t next_event()
     return (*t_events)[t_events_used++];
 }
 
-int64_t g_bounds_bytes = 1ll << 30;   // bounds produced per chunk of reads (mss_set_two_pass_chunk_bytes: tests use small values)
+thread_local int64_t g_bounds_bytes = 256ll << 20;   // bounds produced per chunk of reads (mss_set_two_pass_chunk_bytes: tests use small values)
 
 int32_t two_pass_chunk(const mss_genome* g, int32_t n_reads, int32_t strands)
 {
@@ -493,18 +493,22 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
     int32_t fgrid = 0, fsmem = 0, ftile = 0;
     t_events_used = 0;
     for (int32_t c0 = 0; c0 < p0.n_reads; c0 += chunk) {
-        cudaEvent_t ev0 = t_time_passes ? next_event() : nullptr, ev1 = t_time_passes ? next_event() : nullptr,
-                    ev2 = t_time_passes ? next_event() : nullptr;
-        if (ev0) cudaEventRecord(ev0, st);
+        cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
+        cudaError_t e;
+        if (t_time_passes) {
+            ev0 = next_event(); ev1 = next_event(); ev2 = next_event();
+            if (!ev0 || !ev1 || !ev2) { t_events_used = 0; return cudaErrorMemoryAllocation; }
+            if ((e = cudaEventRecord(ev0, st)) != cudaSuccess) { t_events_used = 0; return e; }
+        }
         ScanParams p = p0;
         p.n_reads = p0.n_reads - c0 < chunk ? p0.n_reads - c0 : chunk;
         p.reads = p0.reads + (int64_t)c0 * p0.stride_words;
         p.reads_nmask = p0.reads_nmask ? p0.reads_nmask + (int64_t)c0 * ((p0.stride_words + 1) / 2) : nullptr;
         p.lens = p0.lens + c0;
         p.ubound = nullptr;
-        cudaError_t e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile);
+        e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile);
         if (e != cudaSuccess) return e;
-        if (ev1) cudaEventRecord(ev1, st);
+        if (ev1 && (e = cudaEventRecord(ev1, st)) != cudaSuccess) { t_events_used = 0; return e; }
         // pass 2: one read per block, every fragment range in one block (the bounds row decides what is scanned)
         p.ubound = ubound;
         p.delta = scan_filter_delta(p);
@@ -518,7 +522,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
             default: e = launch_variant<8, 256>(g, p, ug, out, st, nullptr, 2); break;
         }
         if (e != cudaSuccess) return e;
-        if (ev2) cudaEventRecord(ev2, st);
+        if (ev2 && (e = cudaEventRecord(ev2, st)) != cudaSuccess) { t_events_used = 0; return e; }
         launches += 2;
     }
     if (info) {
@@ -528,9 +532,16 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
     return cudaSuccess;
 }
 
-void scan_set_two_pass_chunk_bytes(int64_t bytes) { g_bounds_bytes = bytes < 1 ? (1ll << 30) : bytes; }
+void scan_set_two_pass_chunk_bytes(int64_t bytes) { g_bounds_bytes = bytes < 1 ? (256ll << 20) : bytes; }
 
-void scan_set_pass_timing(bool on) { t_time_passes = on; if (!on) t_events_used = 0; }
+void scan_set_pass_timing(bool on)
+{
+    t_time_passes = on;
+    if (!on) {                                                  // the events live only while timing is on
+        t_events_used = 0;
+        if (t_events) { for (cudaEvent_t ev : *t_events) cudaEventDestroy(ev); delete t_events; t_events = nullptr; }
+    }
+}
 
 // sums over the chunks of the last two-pass call on this thread; synchronises on its last event
 cudaError_t scan_get_pass_times(float* pass1_ms, float* pass2_ms)

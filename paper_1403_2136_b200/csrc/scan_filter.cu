@@ -201,7 +201,7 @@ FSmem filter_smem(int half, int nw, int32_t max_len, int32_t istep)
 }
 
 // the tile with the least padding among those that leave room for two blocks per SM; -1 = none
-int g_filter_force = -1;      // tuning hook (mss_set_scan_variant 8..12): force one pass-1 tile geometry
+thread_local int g_filter_force = -1;      // tuning hook (mss_set_scan_variant 8..12): force one pass-1 tile geometry
 
 int pick_filter_variant(const mss_genome* g, const ScanParams& p)
 {

@@ -61,22 +61,3 @@ def test_tiny_windows_and_genome_edges(oracle_mod):
     _check(oracle_mod, g, 64, -1, reads, lens)
     _check(oracle_mod, g, 16, 0, reads, lens, pad=0)       # window shorter than the read: forced insertions
     _check(oracle_mod, g, 300, -1, reads, lens)
-
-
-def test_mapq_filter(oracle_mod):
-    import torch
-    import paper_1403_2136_b200 as mss
-    hits = np.array([[[3, 1, 100, 0], [5, 2, 89, 0]],
-                     [[3, 1, 100, 0], [5, 2, 90, 1]],
-                     [[3, 1, 100, 0], [-1, 0, 0, 0]],
-                     [[-1, 0, 0, 0], [-1, 0, 0, 0]],
-                     [[0, 0, 0, 0], [1, 0, 0, 0]],
-                     [[2, 9, 200, 1], [7, 0, 130, 0]]], dtype=np.int32)
-    d = torch.from_numpy(hits).cuda()
-    mapped, mapq = mss.mss_mapq_filter(d, -1.0)
-    assert mapped.cpu().tolist() == [1, 0, 1, 0, 0, 1]       # 10*second < 9*best (ratio below .9)
-    q = mapq.cpu().numpy()
-    assert abs(q[0] + 100 * np.log2(0.89)) < 1e-3 and abs(q[1] - 15.2) < 0.01    # -100 log2 .9 = 15.2
-    mapped62, _ = mss.mss_mapq_filter(d, 62.0)                                     # stricter threshold 62
-    assert mapped62.cpu().tolist() == [0, 0, 1, 0, 0, 1]
-    assert abs(q[5] + 100 * np.log2(0.65)) < 1e-3
