@@ -238,8 +238,10 @@ int mss_version(void);                         /* 100*major + minor */
 /*
  * Tuning / introspection (does not change results): select the scan kernel variant (0 = automatic: the two-pass scan
  * where the geometry allows it, else the one-pass tile kernel, else the generic kernel; 1 = generic; 2-6 = one-pass tile
- * kernels (K, T) = (8,256), (8,128), (8,64), (4,256), (16,128); 7 = two-pass, same as automatic; 8-12 = two-pass with
- * the pass-1 tile (K, T) = (4,256), (4,128), (4,64), (8,128), (8,256) forced; anything else: MSS_ERR_ARG) and report the
+ * kernels (K, T) = (8,256), (8,128), (8,64), (4,256), (16,128); 7 = two-pass, same as automatic: pass 1 is the
+ * lane-per-query kernel for reads of up to 512 scored positions, else the tile kernel; 8-12 = two-pass with pass 1 = the
+ * tile kernel and its tile (K, T) = (4,256), (4,128), (4,64), (8,128), (8,256) forced; 13 = two-pass with the tile kernel
+ * and its own choice of tile; anything else: MSS_ERR_ARG) and report the
  * launch geometry of the last mss_map_reads call on this thread (two-pass: variant 7, grid / smem_bytes / tile_diagonals of
  * pass 1, block 0, launches = 2 per chunk of reads).  Used by bench.py and the parity tests to cover every variant.
  * Every tuning switch of this section (scan variant, forced pass-1 tile, pass timing, bounds chunk size, queries per
@@ -259,6 +261,15 @@ int mss_set_pass_timing(int on);
 /* Bytes of pass-1 bounds produced per chunk of reads (default 256 MiB, <= 0 restores it; this thread only).  The workspace
  * queries follow it.  Results do not depend on it; tests set it small to exercise the chunk loop. */
 int mss_set_two_pass_chunk_bytes(int64_t bytes);
+/* Geometry of the lane-per-query pass-1 kernel (this thread only; results do not depend on it).  query_sets: 32-query
+ * sets per block, 1, 2 or 4 (reads per block = 16, 32 or 64 with both strands, twice that with one; 0 = default 1) --
+ * BASELINE.json config 5's "reads-per-block swept".  tile_window_starts: window starts per tile (even; 0 = automatic:
+ * the tile with the least padding of the fragment length that leaves room for two blocks per SM); a value no tile can
+ * take makes pass 1 fall back to the tile kernel.  arithmetic: how the chains are computed -- 0 = packed int16 DPX
+ * (VIADDMNMX.S16x2.RELU), 1 = fp16 pairs (HFMA2.RELU; exact, every value is an integer <= 2048), 2 = e5m2 operand bytes
+ * widened to fp16 pairs (half the shared-memory traffic), -1 = automatic: the highest of these the scoring and the read
+ * length allow (a forced value that they do not allow is lowered the same way).  Bad values: MSS_ERR_ARG. */
+int mss_set_pass1_geometry(int32_t query_sets, int32_t tile_window_starts, int32_t arithmetic);
 int mss_get_pass_times(float *h_pass1_ms, float *h_pass2_ms);
 
 /*

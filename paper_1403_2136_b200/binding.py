@@ -82,6 +82,7 @@ def lib() -> C.CDLL:
     L.mss_mapq_filter.argtypes = [vp, i32, C.c_double, vp, vp, vp]; L.mss_mapq_filter.restype = C.c_int
     L.mss_set_two_pass_chunk_bytes.argtypes = [C.c_int64]; L.mss_set_two_pass_chunk_bytes.restype = C.c_int
     L.mss_set_pass_timing.argtypes = [C.c_int]; L.mss_set_pass_timing.restype = C.c_int
+    L.mss_set_pass1_geometry.argtypes = [i32, i32, i32]; L.mss_set_pass1_geometry.restype = C.c_int
     L.mss_get_pass_times.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]; L.mss_get_pass_times.restype = C.c_int
     L.mss_map_reads_bounds.argtypes = [vp, vp, vp, i32, vp, i32, i32, _Scoring, i32, i32, vp, vp, C.POINTER(i32)]
     L.mss_map_reads_bounds.restype = C.c_int
@@ -368,6 +369,10 @@ def mss_mapq_filter(d_hits, mapq_threshold: float = -1.0, stream=None):
 
 def mss_set_two_pass_chunk_bytes(nbytes: int) -> None:
     _check(lib().mss_set_two_pass_chunk_bytes(int(nbytes)), "mss_set_two_pass_chunk_bytes")
+
+
+def mss_set_pass1_geometry(query_sets: int = 0, tile_window_starts: int = 0, arithmetic: int = -1) -> None:
+    _check(lib().mss_set_pass1_geometry(int(query_sets), int(tile_window_starts), int(arithmetic)), "mss_set_pass1_geometry")
 
 
 def mss_set_pass_timing(on: bool) -> None:

@@ -161,7 +161,7 @@ int mss_map_reads_bounds(const mss_genome_t* g, const uint32_t* d_reads, const u
     p.istep = every_other ? 2 : 1; p.pssm = nullptr; p.pssm_stride = 0; p.ubound = nullptr; p.delta = 0;
     if (!scan_filter_supported(g, p)) return MSS_ERR_RANGE;
     if (h_delta) *h_delta = scan_filter_delta(p);
-    cudaError_t e = launch_scan_filter(g, p, d_bounds, (cudaStream_t)stream, nullptr, nullptr, nullptr);
+    cudaError_t e = launch_scan_filter(g, p, d_bounds, (cudaStream_t)stream, nullptr, nullptr, nullptr, nullptr);
     if (e != cudaSuccess) return cuda_fail(e);
     return MSS_OK;
 }
@@ -384,11 +384,21 @@ int mss_version(void) { return 100; }
 
 int mss_set_scan_variant(int variant)
 {
-    if (variant < 0 || variant > 12) return MSS_ERR_ARG;
-    // 8..12: the two-pass scan with one pass-1 tile geometry forced (tuning); otherwise pass 1 picks its own
-    scan_filter_force_variant(variant >= 8 && variant <= 12 ? variant - 8 : -1);
-    if (variant >= 8 && variant <= 12) variant = 7;
+    if (variant < 0 || variant > 13) return MSS_ERR_ARG;
+    // 7: the two-pass scan, pass 1 picks its kernel and tile; 8..12: pass 1 = the tile kernel of scan_filter.cu with one tile
+    // geometry forced; 13: the tile kernel with its own choice of tile (tuning and cross-checks)
+    scan_filter_force_variant(variant >= 8 && variant <= 12 ? variant - 8 : -1, variant >= 8);
+    if (variant >= 8) variant = 7;
     t_variant = variant;
+    return MSS_OK;
+}
+
+int mss_set_pass1_geometry(int32_t query_sets, int32_t tile_window_starts, int32_t arithmetic)
+{
+    if (!(query_sets == 0 || query_sets == 1 || query_sets == 2 || query_sets == 4)) return MSS_ERR_ARG;
+    if (tile_window_starts < 0 || (tile_window_starts & 1)) return MSS_ERR_ARG;
+    if (arithmetic < -1 || arithmetic > 2) return MSS_ERR_ARG;
+    scan_filter_lq_tune(query_sets, tile_window_starts / 2, arithmetic);
     return MSS_OK;
 }
 

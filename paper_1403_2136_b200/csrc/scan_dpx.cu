@@ -490,7 +490,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
     const int32_t chunk = two_pass_chunk(g, p0.n_reads, p0.strands);
     uint16_t* ubound = (uint16_t*)ws;
     int launches = 0;
-    int32_t fgrid = 0, fsmem = 0, ftile = 0;
+    int32_t fgrid = 0, fsmem = 0, ftile = 0, frpb = 0;
     t_events_used = 0;
     for (int32_t c0 = 0; c0 < p0.n_reads; c0 += chunk) {
         cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
@@ -506,7 +506,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
         p.reads_nmask = p0.reads_nmask ? p0.reads_nmask + (int64_t)c0 * ((p0.stride_words + 1) / 2) : nullptr;
         p.lens = p0.lens + c0;
         p.ubound = nullptr;
-        e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile);
+        e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile, &frpb);
         if (e != cudaSuccess) return e;
         if (ev1 && (e = cudaEventRecord(ev1, st)) != cudaSuccess) { t_events_used = 0; return e; }
         // pass 2: one read per block, every fragment range in one block (the bounds row decides what is scanned)
@@ -527,7 +527,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
     }
     if (info) {
         info->variant = 7; info->grid = fgrid; info->block = 0; info->smem_bytes = fsmem;
-        info->reads_per_block = 32 / ns; info->tile_diagonals = ftile; info->launches = launches;
+        info->reads_per_block = frpb; info->tile_diagonals = ftile; info->launches = launches;
     }
     return cudaSuccess;
 }

@@ -202,6 +202,7 @@ FSmem filter_smem(int half, int nw, int32_t max_len, int32_t istep)
 
 // the tile with the least padding among those that leave room for two blocks per SM; -1 = none
 thread_local int g_filter_force = -1;      // tuning hook (mss_set_scan_variant 8..12): force one pass-1 tile geometry
+thread_local bool g_filter_tile_kernel = false;   // mss_set_scan_variant 8..13: this file's kernel even where the lane-per-query one applies
 
 int pick_filter_variant(const mss_genome* g, const ScanParams& p)
 {
@@ -253,13 +254,14 @@ cudaError_t launch_filter_variant(const mss_genome* g, const ScanParams& p, uint
 
 }  // namespace
 
-void scan_filter_force_variant(int v) { g_filter_force = v; }
+void scan_filter_force_variant(int v, bool tile_kernel) { g_filter_force = v; g_filter_tile_kernel = tile_kernel; }
 
 bool scan_filter_supported(const mss_genome* g, const ScanParams& p)
 {
     if (p.pssm) return false;                                   // position-specific scores: one-pass scan only
     if (g->frag_len < 256 || g->n_frag < 8) return false;       // nothing to prune
     if ((int64_t)p.max_len * p.match > 32767 || 2 * (int64_t)p.mismatch < -32768 || 2 * (int64_t)p.match > 32767) return false;
+    if (!g_filter_tile_kernel && scan_filter_lq_supported(g, p)) return true;
     return pick_filter_variant(g, p) >= 0;
 }
 
@@ -270,11 +272,14 @@ int32_t scan_filter_delta(const ScanParams& p)
 }
 
 cudaError_t launch_scan_filter(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
-                               int32_t* smem_out, int32_t* tile_out)
+                               int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out)
 {
+    if (!g_filter_tile_kernel && scan_filter_lq_supported(g, p))
+        return launch_scan_filter_lq(g, p, ubound, st, grid_out, smem_out, tile_out, rpb_out);
     int v = pick_filter_variant(g, p);
     if (v < 0) return cudaErrorInvalidConfiguration;
     if (tile_out) *tile_out = 2 * kFVariants[v].K * kFVariants[v].T;
+    if (rpb_out) *rpb_out = FQ_MAX / (p.strands == 3 ? 2 : 1);
     switch (v) {
         case 0: return launch_filter_variant<4, 256>(g, p, ubound, st, grid_out, smem_out);
         case 1: return launch_filter_variant<4, 128>(g, p, ubound, st, grid_out, smem_out);

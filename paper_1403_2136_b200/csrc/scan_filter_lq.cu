@@ -1,0 +1,478 @@
+// Two-pass MaxSS scan, pass 1, lane-per-query layout: the same bounded-error double-step recurrence as
+// scan_filter.cu (G2 = max(G + s1 + s2, 0) sampled every second scored read position; bounds
+// Bt <= best <= Bt + delta), with the roles of the warp lanes turned round:
+//
+//   scan_filter_kernel     lane <-> window start; the query is block-uniform, so the plane offset of every double step is
+//                          a broadcast LDS.128 from a per-query table (one shared-memory wavefront in eight) and the
+//                          fragment maximum of a query needs a warp REDUX per (query, tile, warp)
+//   scan_filter_lq_kernel  lane <-> query (32 queries = 16 reads x 2 strands per warp); the window start is warp-uniform.
+//                          A thread keeps its own query's plane offsets IN REGISTERS for the whole kernel (one per double
+//                          step, or two 16-bit offsets per register for long reads), so a double step of a chain is one
+//                          shared-memory load and one add-max-relu (+ half a 3-input max): no offset loads, no address
+//                          arithmetic, and the maximum over window starts is a per-thread running max: no REDUX.
+//
+// Shared-memory access: the 32 lanes of a warp read the same column of up to 21 different planes.  The plane stride is
+// 1 (mod 32) words, so plane p, word c lies in bank (p + c) mod 32: lanes on different planes hit different banks, lanes
+// on the same plane read the same word (broadcast) -- one wavefront per LDS.32.
+//
+// A warp walks its share of the tile's columns in groups of K = 8 adjacent columns (8 independent chains per thread, each
+// a packed pair of window starts x and x + HALF); the group base is warp-uniform.
+//
+// Arithmetic of the chains (template MODE; all three give the same integers, tests compare them):
+//   LQ_S16   planes hold packed int16 pairs; step = VIADDMNMX.S16x2.RELU (ALU pipe), max = VIMNMX3.S16x2 (ALU pipe).
+//   LQ_F16   planes hold the same integers as fp16 pairs (exact: every value is an integer of magnitude <= 2048); step =
+//            HFMA2.RELU (H * 1 + a, FMA pipe), max = VIMNMX3.S16x2 on the fp16 bit patterns (non-negative fp16 values
+//            order like integers).  The ALU pipe, which the integer form loads to 75 %, only carries the max.
+//   LQ_F8    planes hold e5m2 bytes (= the high byte of the fp16 value; the scores of the default 5/-4 scoring and of
+//            any scoring whose sums have <= 3 significant bits are exact), four per word = two adjacent columns x two
+//            window starts: one LDS.32 feeds two chains, a PRMT per chain widens a byte pair to fp16x2, then as LQ_F16.
+//            Half the shared-memory wavefronts per cell.
+#include <cuda_fp16.h>
+#include "mss_common.cuh"
+
+namespace {
+
+constexpr int LQ_NW = 8;            // warps per block
+constexpr int LQ_K = 8;             // adjacent columns (chains) per thread and column group
+constexpr int LQ_NPL = 21;          // 16 dibase planes + 4 (c1, pad) planes + the all-zero plane of padding steps
+constexpr int LQ_ZERO_PLANE = 20;
+constexpr int LQ_MAX_QSETS = 4;
+enum { LQ_S16 = 0, LQ_F16 = 1, LQ_F8 = 2 };
+
+struct LqGeom {
+    int32_t n_groups, n_splits, frags_per_split, reads_per_group;
+    int32_t qsets;                  // query sets (of 32 lanes) per block: 1, 2 or 4; a set is scanned by NW / qsets warps
+    int32_t HALF, ROWW, NG;         // tile = 2*HALF window starts; plane stride (words); column groups per warp and tile
+    int32_t COLS;                   // columns staged per tile (HALF + look-ahead)
+    int32_t NRAW;                   // packed genome words a tile reads (even)
+};
+
+__device__ __forceinline__ void lq_cp_async4(void* smem_dst, const void* gmem_src)
+{
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(d), "l"(gmem_src) : "memory");
+}
+
+template <int MODE>
+__device__ __forceinline__ uint32_t lq_enc(int32_t v)            // one lane's operand: int16, or fp16 bits of the integer
+{
+    if (MODE == LQ_S16) return (uint32_t)v & 0xFFFFu;
+    return (uint32_t)__half_as_ushort(__int2half_rn(v));
+}
+
+// NJ     = most double steps of a query this instantiation holds (even)
+// PACKED = two 16-bit word offsets per register (long reads) instead of one byte offset per register
+template <int NJ, bool PACKED, int MODE>
+__global__ void __launch_bounds__(32 * LQ_NW, 2)
+scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
+{
+    constexpr int K = LQ_K, NW = LQ_NW, T = 32 * NW;
+    constexpr int NREG = PACKED ? NJ / 2 : NJ;
+    extern __shared__ __align__(16) uint32_t smem[];
+    const int32_t ROWW = ug.ROWW, HALF = ug.HALF, D = 2 * ug.HALF;
+    uint32_t* planes = smem;                                    // LQ_NPL * ROWW
+    uint32_t* wres = planes + LQ_NPL * ROWW;                    // NW * 32: per (warp, lane) tile maximum
+    int32_t* qnj = (int32_t*)(wres + NW * 32);                  // 32 * qsets: double steps of a query; 0 = not scanned
+    int32_t* qm = qnj + 32 * LQ_MAX_QSETS;                      // 32 * qsets: read length
+    uint32_t* rawp = (uint32_t*)(qm + 32 * LQ_MAX_QSETS);       // 2 * NRAW: packed genome words of this tile / the next (cp.async)
+    uint32_t* rawn = rawp + 2 * ug.NRAW;                        // 2 * (NRAW / 2 + 1): N-mask words
+    const int32_t words_before = LQ_NPL * ROWW + NW * 32 + 2 * 32 * LQ_MAX_QSETS + 2 * ug.NRAW + 2 * (ug.NRAW / 2 + 1);
+    uint8_t* codes = reinterpret_cast<uint8_t*>(smem + ((words_before + 3) & ~3));   // 16 * NRAW one-hot base codes (16-byte aligned)
+    uint8_t* sq = reinterpret_cast<uint8_t*>(planes);           // prologue only: strand-oriented base codes, row = query
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int32_t group = blockIdx.x % ug.n_groups, split = blockIdx.x / ug.n_groups;
+    const int32_t ns = (p.strands == 3) ? 2 : 1;
+    const int32_t r0 = group * ug.reads_per_group;
+    const int32_t nr = min(ug.reads_per_group, p.n_reads - r0);
+    const int32_t nq = nr * ns;
+    const int32_t f_begin = split * ug.frags_per_split;
+    const int32_t f_end = min(p.n_frag, f_begin + ug.frags_per_split);
+    const int32_t istep = p.istep;
+    const int32_t wps = NW / ug.qsets;                          // warps per query set
+    const int32_t set = warp / wps, ws = warp % wps;
+    const int32_t CW = HALF / wps;                              // columns of a tile scanned by one warp
+    const int32_t sq_stride = (p.max_len + 3) & ~3;
+
+    // ---- a1 read prep, step 1: strand-oriented base codes of every query of the block (bytes; 4 = N) -----------------
+    for (int32_t q = warp; q < 32 * ug.qsets; q += NW) {
+        int32_t njq = 0, m = 0;
+        if (q < nq) {
+            const int32_t r = r0 + q / ns;
+            const int32_t strand = (ns == 2) ? (q & 1) : (p.strands == 2 ? 1 : 0);
+            m = p.lens[r];
+            const bool ok = (m >= 1 && m <= p.max_len);
+            const uint32_t* rw = p.reads + (int64_t)r * p.stride_words;
+            const uint32_t* rn = p.reads_nmask ? p.reads_nmask + (int64_t)r * ((p.stride_words + 1) / 2) : nullptr;
+            bool has_n = false;
+            if (ok) {
+                for (int32_t i = lane; i < m; i += 32) {
+                    uint32_t b = read_base(rw, rn, m, i, strand);
+                    if (b == 4u && i % istep == 0) has_n = true;        // only scored positions matter
+                    sq[q * sq_stride + i] = (uint8_t)b;
+                }
+            }
+            has_n = __any_sync(0xffffffffu, has_n);
+            const int32_t steps = ok ? (m + istep - 1) / istep : 0;
+            njq = (ok && !has_n) ? (steps + 1) / 2 : 0;             // a query holding an N is not scanned: bound 0xFFFF
+        }
+        if (lane == 0) { qnj[q] = njq; qm[q] = m; }
+    }
+    __syncthreads();
+
+    // ---- step 2: this lane's query -> plane offsets in registers -----------------------------------------------------
+    // a column is a word (LQ_S16, LQ_F16) or half a word (LQ_F8: columns 2c, 2c+1 share word c; every offset below is even)
+    const int32_t myq = set * 32 + lane;
+    const int32_t mynj = qnj[myq], mym = qm[myq];
+    uint32_t off[NREG];
+#pragma unroll
+    for (int j = 0; j < NJ; j++) {
+        uint32_t plane = LQ_ZERO_PLANE, col = 0u;                   // padding step: adds 0
+        if (j < mynj) {
+            const int32_t i1 = 2 * j * istep, i2 = i1 + istep;
+            const uint32_t b1 = sq[myq * sq_stride + i1];
+            const uint32_t b2 = (i2 < mym) ? sq[myq * sq_stride + i2] : 4u;     // 4 = past the end: the (c1, pad) plane
+            plane = b1 * 5u + b2; col = (uint32_t)i1;
+        }
+        const uint32_t cw = col + (uint32_t)(ws * CW);              // column of chain 0, group 0
+        const uint32_t w = plane * (uint32_t)ROWW + (MODE == LQ_F8 ? cw >> 1 : cw);
+        if (PACKED) {
+            if (j & 1) off[j >> 1] |= w << 16; else off[j >> 1] = w;
+        } else {
+            asm("shl.b32 %0, %1, 2;" : "=r"(off[j]) : "r"(w));     // opaque: keeps ptxas from storing w and re-scaling it (LEA) per use
+        }
+    }
+    // double steps this warp runs: the longest query of its set, rounded up to the pair the loop body handles
+    const int32_t njb = (__reduce_max_sync(0xffffffffu, mynj) + 1) & ~1;
+
+    const uint32_t zero = (uint32_t)p.zero;
+    const int32_t tiles_per_frag = (p.F + D - 1) / D;
+    const int32_t M = p.match, X = p.mismatch;
+    // encodings of the five possible operands: a double step scores 0, 1 or 2 matches, a single step 0 or 1
+    const uint32_t e2_0 = lq_enc<MODE>(2 * X), e2_1 = lq_enc<MODE>(M + X), e2_2 = lq_enc<MODE>(2 * M);
+    const uint32_t e1_0 = lq_enc<MODE>(X), e1_1 = lq_enc<MODE>(M);
+    const char* planes_b = reinterpret_cast<const char*>(planes);
+    uint32_t cur = 0u;                                              // fold threads (tid < 32 * qsets): running fragment maximum
+    int32_t prev_f = -1; bool prev_last = false;
+
+    auto fold = [&]() {                                             // previous tile's per-warp maxima -> fragment maximum -> bound
+        if (prev_f < 0 || tid >= 32 * ug.qsets) return;
+        // thread tid < 32*qsets folds query tid: its set is tid / 32, scanned by warps [set*wps, (set+1)*wps)
+        const int32_t fs = tid >> 5;
+        uint32_t c = cur;
+        for (int32_t w = 0; w < wps; w++) c = max(c, wres[(fs * wps + w) * 32 + lane]);
+        if (prev_last) {
+            if (tid < nq) {
+                const int32_t r = r0 + tid / ns, s = tid % ns;
+                uint32_t u = c;                                     // fp16 modes: bit pattern of a non-negative integer value
+                if (MODE != LQ_S16) u = (uint32_t)__half2int_rn(__ushort_as_half((unsigned short)c));
+                ubound[((int64_t)r * ns + s) * p.n_frag + prev_f] = (qnj[tid] == 0) ? (uint16_t)0xFFFFu : (uint16_t)u;
+            }
+            c = 0u;
+        }
+        cur = c;
+    };
+
+    // ---- a2, asynchronous half: the raw 2-bit words and N-mask words of a tile travel to shared memory by cp.async
+    // (LDGSTS) one tile ahead of the scan; raw word i of a tile is packed word w0 + i, w0 = g0 / 16
+    const int32_t n_tiles = (f_end - f_begin) * tiles_per_frag;
+    auto prefetch = [&](int32_t it) {
+        const int32_t f = f_begin + it / tiles_per_frag, tile = it % tiles_per_frag;
+        const int64_t g0 = (int64_t)f * p.F + (int64_t)tile * D;
+        const int64_t w0 = g0 >> 4;
+        uint32_t* rp = rawp + (it & 1) * ug.NRAW;
+        uint32_t* rn = rawn + (it & 1) * (ug.NRAW / 2 + 1);
+        for (int32_t i = tid; i < ug.NRAW; i += T) lq_cp_async4(rp + i, p.gpacked + w0 + i);
+        for (int32_t i = tid; i < ug.NRAW / 2 + 1; i += T) lq_cp_async4(rn + i, p.gnmask + (w0 >> 1) + i);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    if (n_tiles > 0) prefetch(0);
+
+    for (int32_t it = 0; it < n_tiles; it++) {
+        const int32_t f = f_begin + it / tiles_per_frag, tile = it % tiles_per_frag;
+        const int64_t fstart = (int64_t)f * p.F;
+        const int64_t trunc = (p.V < 0) ? (int64_t)0x7FFFFFFFFFFFFFFFll : fstart + p.F + p.V;
+        {
+            const int32_t toff = tile * D;
+            const int64_t g0 = fstart + toff;
+            const int32_t nvalid = min(D, p.F - toff);
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();                                        // previous tile scanned (planes free, wres complete); raw words landed
+            fold();
+            // ---- a2: raw words -> one byte per genome position: one-hot of the base (1, 2, 4, 8), 0 = N or not readable
+            {
+                const uint32_t* rp = rawp + (it & 1) * ug.NRAW;
+                const uint32_t* rn = rawn + (it & 1) * (ug.NRAW / 2 + 1);
+                const int64_t w0 = g0 >> 4;
+                for (int32_t i = tid; i < ug.NRAW; i += T) {
+                    const uint32_t w = rp[i];
+                    const int64_t W = w0 + i;
+                    const uint32_t mk = (rn[(int32_t)((W >> 1) - (w0 >> 1))] >> (16u * (uint32_t)(W & 1))) & 0xFFFFu;
+                    const int64_t pos0 = W << 4;
+                    uint32_t out[4];
+#pragma unroll
+                    for (int b = 0; b < 16; b++) {
+                        const uint32_t c = (w >> (2 * b)) & 3u;
+                        const bool dead = ((mk >> b) & 1u) || (pos0 + b >= trunc);
+                        const uint32_t oh = dead ? 0u : (1u << c);
+                        if ((b & 3) == 0) out[b >> 2] = oh; else out[b >> 2] |= oh << (8 * (b & 3));
+                    }
+                    *reinterpret_cast<uint4*>(codes + 16 * i) = make_uint4(out[0], out[1], out[2], out[3]);
+                }
+            }
+            if (it + 1 < n_tiles) prefetch(it + 1);
+            __syncthreads();
+            // ---- a2: codes -> dibase planes ----------------------------------------------------------------------
+            const int32_t sh = (int32_t)(g0 & 15);                  // codes[sh + x] = genome position g0 + x
+            if (MODE != LQ_F8) {
+                for (int32_t x = tid; x < ug.COLS; x += T) {
+                    const uint32_t lo1 = codes[sh + x], lo2 = codes[sh + x + istep];
+                    const uint32_t hi1 = codes[sh + x + HALF], hi2 = codes[sh + x + HALF + istep];
+#pragma unroll
+                    for (uint32_t c1 = 0; c1 < 4; c1++) {
+                        const uint32_t ml = (lo1 >> c1) & 1u, mh = (hi1 >> c1) & 1u;
+#pragma unroll
+                        for (uint32_t c2 = 0; c2 < 4; c2++) {
+                            const uint32_t nl = ml + ((lo2 >> c2) & 1u), nh = mh + ((hi2 >> c2) & 1u);
+                            const uint32_t vl = nl == 2 ? e2_2 : (nl == 1 ? e2_1 : e2_0), vh = nh == 2 ? e2_2 : (nh == 1 ? e2_1 : e2_0);
+                            planes[(c1 * 5 + c2) * ROWW + x] = vl | (vh << 16);
+                        }
+                        planes[(c1 * 5 + 4) * ROWW + x] = (ml ? e1_1 : e1_0) | ((mh ? e1_1 : e1_0) << 16);
+                    }
+                    planes[LQ_ZERO_PLANE * ROWW + x] = 0u;
+                }
+            } else {
+                // word xw = columns 2xw, 2xw + 1, bytes (lo, hi, lo', hi').  The four lanes' one-hot codes go into the four
+                // nibbles of a 16-bit value; (OH >> c) & 0x1111 is then the lanes' match flag against base c, the sum of two
+                // such values their match count (0..2 per nibble), and one PRMT with that value as the selector maps every
+                // count to its operand byte: 3 instructions per plane word
+                const uint32_t tab2 = (e2_0 >> 8) | (e2_1 & 0xFF00u) | ((e2_2 & 0xFF00u) << 8);
+                const uint32_t tab1 = (e1_0 >> 8) | (e1_1 & 0xFF00u);
+                for (int32_t xw = tid; xw < ug.COLS / 2; xw += T) {
+                    const uint8_t* c0 = codes + sh + 2 * xw;
+                    const uint32_t oh1 = c0[0] | (c0[HALF] << 4) | (c0[1] << 8) | (c0[HALF + 1] << 12);
+                    const uint32_t oh2 = c0[istep] | (c0[HALF + istep] << 4) | (c0[1 + istep] << 8) | (c0[HALF + 1 + istep] << 12);
+                    uint32_t A[4], Bm[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) { A[c] = (oh1 >> c) & 0x1111u; Bm[c] = (oh2 >> c) & 0x1111u; }
+#pragma unroll
+                    for (uint32_t c1 = 0; c1 < 4; c1++) {
+#pragma unroll
+                        for (uint32_t c2 = 0; c2 < 4; c2++)
+                            planes[(c1 * 5 + c2) * ROWW + xw] = __byte_perm(tab2, 0u, A[c1] + Bm[c2]);
+                        planes[(c1 * 5 + 4) * ROWW + xw] = __byte_perm(tab1, 0u, A[c1]);
+                    }
+                    planes[LQ_ZERO_PLANE * ROWW + xw] = 0u;
+                }
+            }
+            __syncthreads();
+
+            // ---- a3: this lane's query against the warp's columns of the tile --------------------------------------
+            uint32_t tmax = 0u;
+            for (int32_t g = 0; g < ug.NG; g++) {
+                const char* pg = planes_b + g * (MODE == LQ_F8 ? K * 2 : K * 4);    // warp-uniform group base
+                uint32_t H[K], B[K];
+#pragma unroll
+                for (int k = 0; k < K; k++) { H[k] = 0u; B[k] = 0u; }
+#pragma unroll
+                for (int j = 0; j < NJ; j += 2) {
+                    if (j >= njb) break;
+                    uint32_t o0, o1;
+                    if (PACKED) {                                   // volatile: unpacked per use, or the compiler hoists all NJ results out of the group loop and spills them
+                        uint32_t lo, hi;
+                        asm volatile("and.b32 %0, %1, 0xFFFF;" : "=r"(lo) : "r"(off[j >> 1]));
+                        asm volatile("shr.u32 %0, %1, 16;" : "=r"(hi) : "r"(off[j >> 1]));
+                        o0 = lo << 2; o1 = hi << 2;
+                    }
+                    else { o0 = off[j]; o1 = off[j + 1]; }
+                    uint32_t Ha[K], v[K];
+                    if (MODE == LQ_F8) {
+#pragma unroll
+                        for (int k = 0; k < K; k += 2) {
+                            const uint32_t w = *reinterpret_cast<const uint32_t*>(pg + o0 + k * 2);
+                            v[k] = __byte_perm(w, 0u, 0x1404); v[k + 1] = __byte_perm(w, 0u, 0x3424);
+                        }
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < K; k++) v[k] = *reinterpret_cast<const uint32_t*>(pg + o0 + k * 4);
+                    }
+#pragma unroll
+                    for (int k = 0; k < K; k++) {
+                        if (MODE == LQ_S16) Ha[k] = __viaddmax_s16x2(H[k], v[k], zero);
+                        else asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(Ha[k]) : "r"(H[k]), "r"(0x3C003C00u), "r"(v[k]));
+                    }
+                    if (MODE == LQ_F8) {
+#pragma unroll
+                        for (int k = 0; k < K; k += 2) {
+                            const uint32_t w = *reinterpret_cast<const uint32_t*>(pg + o1 + k * 2);
+                            v[k] = __byte_perm(w, 0u, 0x1404); v[k + 1] = __byte_perm(w, 0u, 0x3424);
+                        }
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < K; k++) v[k] = *reinterpret_cast<const uint32_t*>(pg + o1 + k * 4);
+                    }
+#pragma unroll
+                    for (int k = 0; k < K; k++) {
+                        if (MODE == LQ_S16) H[k] = __viaddmax_s16x2(Ha[k], v[k], zero);
+                        else asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(H[k]) : "r"(Ha[k]), "r"(0x3C003C00u), "r"(v[k]));
+                    }
+#pragma unroll
+                    for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                }
+                if (nvalid < D) {                                   // ragged last tile of a fragment: drop foreign window starts
+                    const int32_t x0 = ws * CW + g * K;
+#pragma unroll
+                    for (int k = 0; k < K; k++) {
+                        if (x0 + k >= nvalid) B[k] &= 0xFFFF0000u;
+                        if (x0 + k + HALF >= nvalid) B[k] &= 0x0000FFFFu;
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < K; k++) tmax = __vmaxs2(tmax, B[k]);
+            }
+            wres[warp * 32 + lane] = max(tmax & 0xFFFFu, tmax >> 16);
+            prev_f = f; prev_last = (tile == tiles_per_frag - 1);
+        }
+    }
+    __syncthreads();
+    fold();
+}
+
+// every value a plane can hold, as an e5m2 byte (= the high byte of its fp16 form), must be exact
+bool lq_e5m2_exact(int32_t v)
+{
+    if (v < 0) v = -v;
+    if (v == 0) return true;
+    if (v > 57344) return false;                                // the largest finite e5m2 value
+    while ((v & 1) == 0) v >>= 1;
+    return v < 8;                                               // three significant bits (1.xx)
+}
+
+struct LqSmem { int32_t ROWW, COLS, NRAW; size_t bytes; };
+LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode)
+{
+    // columns read: chain column < HALF, plus the column of the last double step (< max_len rounded up to even steps)
+    LqSmem s;
+    int32_t halo = ((max_len + 2 * istep + 3) & ~3);
+    s.COLS = half + halo;
+    int32_t roww = mode == LQ_F8 ? s.COLS / 2 : s.COLS;
+    roww += (33 - (roww & 31)) & 31;                            // 1 (mod 32): plane p, word c -> bank (p + c) mod 32
+    s.ROWW = roww;
+    // genome positions a tile reads: [g0, g0 + HALF + COLS + istep), from the 16-aligned position below g0
+    s.NRAW = ((half + s.COLS + istep + 15 + 15) / 16 + 1) & ~1;
+    // planes, wres, qnj + qm, raw words (2 buffers), raw mask words (2 buffers), pad to 16 bytes, codes
+    size_t words = (size_t)LQ_NPL * roww + LQ_NW * 32 + 2 * 32 * LQ_MAX_QSETS + 2 * s.NRAW + 2 * (s.NRAW / 2 + 1);
+    words = (words + 3) & ~(size_t)3;
+    s.bytes = words * 4 + (size_t)16 * s.NRAW;
+    return s;
+}
+
+thread_local int t_lq_qsets = 1;       // tuning hook: query sets per block (reads per block = 16 * qsets with both strands)
+thread_local int t_lq_half = 0;        // tuning hook: force the tile (0 = automatic)
+thread_local int t_lq_mode = -1;       // tuning hook: force the arithmetic (-1 = automatic)
+
+int lq_mode(const ScanParams& p)
+{
+    const int32_t M = p.match, X = p.mismatch;
+    const bool f16_ok = (int64_t)p.max_len * M <= 2048 && 2 * M <= 2048 && -2 * X <= 2048;
+    const bool f8_ok = f16_ok && lq_e5m2_exact(2 * M) && lq_e5m2_exact(M + X) && lq_e5m2_exact(2 * X) && lq_e5m2_exact(M) &&
+                       lq_e5m2_exact(X);
+    int want = t_lq_mode >= 0 ? t_lq_mode : LQ_F8;
+    if (want == LQ_F8 && !f8_ok) want = LQ_F16;
+    if (want == LQ_F16 && !f16_ok) want = LQ_S16;
+    return want;
+}
+
+// the tile: 2*HALF window starts, HALF a multiple of the columns one more group of every warp of a set adds;
+// least padding of the fragment length first, larger tiles on ties; two blocks per SM must fit
+bool lq_pick(const mss_genome* g, const ScanParams& p, int32_t qsets, int mode, LqGeom* out)
+{
+    const int32_t unit = (LQ_NW / qsets) * LQ_K;
+    const size_t prologue = (size_t)32 * qsets * ((p.max_len + 3) & ~3);
+    int32_t best = 0; double best_waste = 1e30;
+    for (int32_t half = unit; half <= 4096; half += unit) {
+        if (t_lq_half > 0 && half != t_lq_half) continue;
+        if (half < 128) continue;
+        LqSmem s = lq_smem(half, p.max_len, p.istep, mode);
+        if (s.bytes * 2 + 4096 > (size_t)g->max_smem_optin) break;
+        if ((size_t)LQ_NPL * s.ROWW * 4 < prologue) continue;      // the prologue borrows the plane area
+        if ((int64_t)LQ_NPL * s.ROWW + 4096 > 65535) break;          // packed 16-bit word offsets
+        int32_t D = 2 * half;
+        double waste = (double)((g->frag_len + D - 1) / D) * D / g->frag_len;
+        waste *= 1.0 + 0.02 * (double)(s.COLS - half) / half;       // look-ahead columns are staged, not scanned: mild preference for large tiles
+        if (waste < best_waste - 1e-9) { best_waste = waste; best = half; }
+    }
+    if (!best) return false;
+    if (out) {
+        LqSmem s = lq_smem(best, p.max_len, p.istep, mode);
+        out->HALF = best; out->ROWW = s.ROWW; out->COLS = s.COLS; out->NRAW = s.NRAW; out->qsets = qsets; out->NG = best / unit;
+    }
+    return true;
+}
+
+int32_t lq_double_steps(const ScanParams& p)
+{
+    int32_t steps = (p.max_len + p.istep - 1) / p.istep;
+    return (steps + 1) / 2;
+}
+
+template <int NJ, bool PACKED, int MODE>
+cudaError_t lq_launch3(const ScanParams& p, const LqGeom& ug, uint16_t* ubound, cudaStream_t st, size_t smem)
+{
+    cudaError_t e = cudaFuncSetAttribute(scan_filter_lq_kernel<NJ, PACKED, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int64_t blocks = (int64_t)ug.n_groups * ug.n_splits;
+    scan_filter_lq_kernel<NJ, PACKED, MODE><<<(unsigned)blocks, 32 * LQ_NW, smem, st>>>(p, ug, ubound);
+    return cudaGetLastError();
+}
+
+template <int NJ, bool PACKED>
+cudaError_t lq_launch(int mode, const ScanParams& p, const LqGeom& ug, uint16_t* ubound, cudaStream_t st, size_t smem)
+{
+    if (mode == LQ_F8) return lq_launch3<NJ, PACKED, LQ_F8>(p, ug, ubound, st, smem);
+    if (mode == LQ_F16) return lq_launch3<NJ, PACKED, LQ_F16>(p, ug, ubound, st, smem);
+    return lq_launch3<NJ, PACKED, LQ_S16>(p, ug, ubound, st, smem);
+}
+
+}  // namespace
+
+void scan_filter_lq_tune(int qsets, int half, int mode)
+{
+    t_lq_qsets = (qsets == 2 || qsets == 4) ? qsets : 1;
+    t_lq_half = half > 0 ? half : 0;
+    t_lq_mode = (mode >= 0 && mode <= 2) ? mode : -1;
+}
+
+bool scan_filter_lq_supported(const mss_genome* g, const ScanParams& p)
+{
+    if (lq_double_steps(p) > 128) return false;                 // longer queries: the tile kernel of scan_filter.cu
+    return lq_pick(g, p, t_lq_qsets, lq_mode(p), nullptr);
+}
+
+cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
+                                  int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out)
+{
+    LqGeom ug;
+    const int mode = lq_mode(p);
+    if (!lq_pick(g, p, t_lq_qsets, mode, &ug)) return cudaErrorInvalidConfiguration;
+    const int32_t ns = p.strands == 3 ? 2 : 1;
+    ug.reads_per_group = 32 * ug.qsets / ns;
+    ug.n_groups = (p.n_reads + ug.reads_per_group - 1) / ug.reads_per_group;
+    if (ug.n_groups < 1) ug.n_groups = 1;
+    int64_t target = (int64_t)g->sm_count * 2 * 48;             // ~48 waves of the 2 resident blocks per SM
+    int64_t want = (target + ug.n_groups - 1) / ug.n_groups;
+    if (want < 1) want = 1;
+    if (want > g->n_frag) want = g->n_frag;
+    ug.frags_per_split = (int32_t)((g->n_frag + want - 1) / want);
+    ug.n_splits = (g->n_frag + ug.frags_per_split - 1) / ug.frags_per_split;
+    const size_t smem = lq_smem(ug.HALF, p.max_len, p.istep, mode).bytes;
+    if (grid_out) *grid_out = (int32_t)((int64_t)ug.n_groups * ug.n_splits);
+    if (smem_out) *smem_out = (int32_t)smem;
+    if (tile_out) *tile_out = 2 * ug.HALF;
+    if (rpb_out) *rpb_out = ug.reads_per_group;
+    const int32_t nj = lq_double_steps(p);
+    if (nj <= 32) return lq_launch<32, false>(mode, p, ug, ubound, st, smem);
+    if (nj <= 64) return lq_launch<64, false>(mode, p, ug, ubound, st, smem);
+    if (nj <= 80) return lq_launch<80, false>(mode, p, ug, ubound, st, smem);
+    return lq_launch<128, true>(mode, p, ug, ubound, st, smem);
+}

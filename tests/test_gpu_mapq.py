@@ -69,7 +69,8 @@ def test_mapq_single_fragment_and_zero_scores(oracle_mod):
     import paper_1403_2136_b200 as mss
     from gpu_util import load_genome, to_dev
     g = gen.make_genome(3000, 61)[0]
-    g[g == 0] = 1                                          # no A in the genome
+    g[g == 0] = 1                                          # no A and no T in the genome: an all-A read scores 0 on
+    g[g == 3] = 2                                          # both strands (its reverse complement is all T)
     reads = np.stack([g[500:560], gen.revcomp(g[900:960]), np.zeros(60, dtype=np.uint8)])
     lens = np.full(3, 60, dtype=np.int32)
     G = load_genome(g, 3000, -1)

@@ -15,6 +15,31 @@ def _cmp(got, want, ctx=""):
     assert bad.size == 0, f"{ctx}: {bad.size} reads differ, first {bad[0]}: got {got[bad[0]].tolist()} want {want[bad[0]].tolist()}"
 
 
+# pass-1 kernels and arithmetic: (scan variant, arithmetic of the lane-per-query kernel)
+#   (7, -1) automatic = lane-per-query kernel, e5m2 operand bytes where the scoring allows; (7, 0) packed int16 DPX;
+#   (7, 1) fp16 pairs; (7, 2) e5m2 bytes (lowered where the scoring is not exact in e5m2); (13, -1) the tile kernel
+PASS1 = [(7, -1), (7, 0), (7, 1), (7, 2), (13, -1)]
+
+
+class pass1_setup:
+    """Select the pass-1 kernel for the calls inside the with-block (thread-local switches of the library)."""
+
+    def __init__(self, variant=7, arithmetic=-1, query_sets=0, tile=0):
+        self.args = (variant, arithmetic, query_sets, tile)
+
+    def __enter__(self):
+        import paper_1403_2136_b200 as mss
+        v, a, q, t = self.args
+        mss.mss_set_pass1_geometry(q, t, a)
+        mss.mss_set_scan_variant(v)
+        return self
+
+    def __exit__(self, *exc):
+        import paper_1403_2136_b200 as mss
+        mss.mss_set_pass1_geometry(0, 0, -1)
+        mss.mss_set_scan_variant(0)
+
+
 def _bounds(G, reads, lens, strands, match=5, mismatch=-4, fast=False):
     import torch
     import paper_1403_2136_b200 as mss
@@ -51,6 +76,8 @@ def _exact_fragment_scores(oracle_mod, g, F, V, read, m, strand, match, mismatch
     (1000, -1, 100, 5, -4, True), (1000, 0, 51, 5, -4, True), (1000, -1, 75, 3, -5, True),
 ])
 def test_pass1_bounds_hold(oracle_mod, F, V, m, match, mismatch, fast):
+    """Every pass-1 kernel and arithmetic: u <= exact <= u + delta against the oracle's per-fragment scores; the
+    bounds of the different kernels are the same integers (they compute the same recurrence)."""
     from gpu_util import load_genome
     g = gen.make_genome(40_000, 31)[0]
     g[5000:5300] = gen.N
@@ -59,14 +86,20 @@ def test_pass1_bounds_hold(oracle_mod, F, V, m, match, mismatch, fast):
     lens[5] = max(1, m - 7); reads[5, lens[5]:] = gen.N
     lens[9] = 1; reads[9, 1:] = gen.N
     G = load_genome(g, F, V)
-    u, delta = _bounds(G, reads, lens, 3, match, mismatch, fast)
-    assert delta == min(match, -mismatch) - mismatch
-    for i in range(reads.shape[0]):
-        for s in (0, 1):
-            exact = _exact_fragment_scores(oracle_mod, g, F, V, reads[i], int(lens[i]), s, match, mismatch, fast)
+    exact = {(i, s): _exact_fragment_scores(oracle_mod, g, F, V, reads[i], int(lens[i]), s, match, mismatch, fast)
+             for i in range(reads.shape[0]) for s in (0, 1)}
+    first = None
+    for variant, arith in PASS1:
+        with pass1_setup(variant, arith):
+            u, delta = _bounds(G, reads, lens, 3, match, mismatch, fast)
+        assert delta == min(match, -mismatch) - mismatch
+        for (i, s), ex in exact.items():
             ui = u[i, s]
             assert (ui != 0xFFFF).all()
-            assert (ui <= exact).all() and (exact <= ui + delta).all(), (i, s, int(np.argmax(np.abs(exact - ui))))
+            assert (ui <= ex).all() and (ex <= ui + delta).all(), (variant, arith, i, s, int(np.argmax(np.abs(ex - ui))))
+        if first is None:
+            first = u
+        assert (u == first).all(), (variant, arith)
 
 
 def test_pass1_marks_reads_with_n_as_unbounded(oracle_mod):
@@ -93,9 +126,57 @@ def test_two_pass_records_equal_oracle(oracle_mod, F, V, strands):
     lens[11] = 99; reads[11, 99:] = gen.N                 # odd length: the last double step has a single position
     G = load_genome(g, F, V)
     want = oracle_mod.map_reads_parallel(g, F, V, reads, lens, strands=strands)
-    _cmp(map_reads(G, reads, lens, strands=strands, variant=7), want, f"two-pass F={F} V={V} strands={strands}")
-    want = oracle_mod.map_reads_parallel(g, F, V, reads, lens, strands=strands, fast=True)
-    _cmp(map_reads_fast(G, reads, lens, strands=strands, variant=7), want, f"two-pass fast F={F} V={V} strands={strands}")
+    want_fast = oracle_mod.map_reads_parallel(g, F, V, reads, lens, strands=strands, fast=True)
+    for variant, arith in PASS1:
+        with pass1_setup(variant, arith):
+            _cmp(map_reads(G, reads, lens, strands=strands, variant=variant), want, f"two-pass {variant}/{arith} F={F} V={V} strands={strands}")
+        with pass1_setup(variant, arith):
+            _cmp(map_reads_fast(G, reads, lens, strands=strands, variant=variant), want_fast,
+                 f"two-pass fast {variant}/{arith} F={F} V={V} strands={strands}")
+
+
+@pytest.mark.parametrize("m", [1, 2, 3, 35, 64, 127, 128, 129, 159, 160, 161, 255, 256, 257, 300])
+def test_two_pass_read_lengths_across_the_register_table_limits(oracle_mod, m):
+    """The lane-per-query pass 1 keeps a query's plane offsets in registers: 32, 64 or 80 double steps directly, up to 128
+    as 16-bit pairs; longer reads take the tile kernel.  Lengths on both sides of every limit, mixed with shorter reads in
+    the same block (padding steps on the all-zero plane), all three arithmetics."""
+    from gpu_util import load_genome, map_reads
+    g = gen.make_genome(30_000, 36)[0]
+    r = gen.make_reads(g, 40, m, 3600 + m, sub_rate=0.12, indel_prob=0.0 if m < 8 else 0.5)
+    reads, lens = r["reads"].copy(), r["lens"].copy()
+    for k, short in ((3, m // 2), (8, m - 1), (20, 1), (21, 2)):
+        if 1 <= short < m:
+            lens[k] = short; reads[k, short:] = gen.N
+    G = load_genome(g, 1536, -1)
+    want = oracle_mod.map_reads_parallel(g, 1536, -1, reads, lens, strands=3)
+    for arith in (0, 1, 2):
+        with pass1_setup(7, arith):
+            _cmp(map_reads(G, reads, lens, strands=3, variant=7), want, f"m={m} arithmetic {arith}")
+
+
+@pytest.mark.parametrize("query_sets,tile", [(1, 0), (2, 0), (4, 0), (1, 512), (2, 1024), (4, 768), (1, 2048)])
+def test_pass1_reads_per_block_and_tile_do_not_change_results(oracle_mod, query_sets, tile):
+    """BASELINE.json config 5's "reads-per-block swept": 16, 32 or 64 reads (x 2 strands) per block, and forced tiles
+    including ragged ones (F = 1000 is not a multiple of any tile), partial last groups (75 reads)."""
+    from gpu_util import load_genome, map_reads
+    import paper_1403_2136_b200 as mss
+    cfg = gen.config(1)
+    g, _ = cfg.genome()
+    r = cfg.reads(g)
+    reads, lens = r["reads"][:75].copy(), r["lens"][:75].copy()
+    reads[1::2] = np.stack([gen.revcomp(x) for x in reads[1::2]])
+    for F in (1000, 4096):
+        G = load_genome(g, F, -1)
+        want = oracle_mod.map_reads_parallel(g, F, -1, reads, lens, strands=3)
+        for strands in (1, 3):
+            w = want if strands == 3 else oracle_mod.map_reads_parallel(g, F, -1, reads, lens, strands=1)
+            with pass1_setup(7, -1, query_sets, tile):
+                got = map_reads(G, reads, lens, strands=strands, variant=7)
+                info = mss.mss_get_last_launch()
+            _cmp(got, w, f"query_sets={query_sets} tile={tile} F={F} strands={strands}")
+            assert info["variant"] == 7 and info["reads_per_block"] == 32 * query_sets // (2 if strands == 3 else 1)
+            if tile:
+                assert info["tile_diagonals"] == tile
 
 
 def test_two_pass_ties_duplicates_and_zero_scores(oracle_mod):
@@ -114,7 +195,9 @@ def test_two_pass_ties_duplicates_and_zero_scores(oracle_mod):
     for genome in (g, gz):
         G = load_genome(genome, 1000, -1)
         want = oracle_mod.map_reads_parallel(genome, 1000, -1, reads, lens, strands=3)
-        _cmp(map_reads(G, reads, lens, strands=3, variant=7), want, "ties")
+        for variant, arith in PASS1:
+            with pass1_setup(variant, arith):
+                _cmp(map_reads(G, reads, lens, strands=3, variant=variant), want, f"ties {variant}/{arith}")
     per = np.tile(np.array([0, 1], dtype=np.uint8), 6000)
     G = load_genome(per, 512, -1)
     rd = np.tile(np.array([0, 1], dtype=np.uint8), 30)[None, :]
@@ -129,7 +212,10 @@ def test_two_pass_other_scorings_and_long_reads(oracle_mod):
     G = load_genome(g, 1500, -1)
     for match, mismatch in ((1, -1), (2, -3), (9, -7), (10, -40), (3, -1)):
         want = oracle_mod.map_reads_parallel(g, 1500, -1, r["reads"], r["lens"], match=match, mismatch=mismatch, strands=3)
-        _cmp(map_reads(G, r["reads"], r["lens"], match=match, mismatch=mismatch, variant=7), want, f"scoring {match}/{mismatch}")
+        for variant, arith in PASS1:
+            with pass1_setup(variant, arith):
+                _cmp(map_reads(G, r["reads"], r["lens"], match=match, mismatch=mismatch, variant=variant), want,
+                     f"scoring {match}/{mismatch} pass 1 {variant}/{arith}")
     r = gen.make_reads(g, 6, 700, 3401, sub_rate=0.1)
     G = load_genome(g, 2048, -1)
     want = oracle_mod.map_reads_parallel(g, 2048, -1, r["reads"], r["lens"], strands=3)
