@@ -26,11 +26,20 @@ sys.path.insert(0, ROOT)
 
 import gen  # noqa: E402
 
-ALGO_INSTR_PER_CELL = 0.75          # one-pass scan: 1 VIADDMNMX.S16x2 per 2 cells + 1 VIMNMX3.S16x2 per 4 cells
-ALGO_INSTR_PER_CELL_PASS1 = 0.375   # two-pass scan, pass 1: 1 VIADDMNMX.S16x2 per 4 cells + 1 VIMNMX3.S16x2 per 8 cells
-NCU_DRAM_BYTES_PASS1 = 2_019_072     # profiles/r1_scan_filter_full.md (2.00 MB read + 0.02 MB written per launch)
-NCU_DRAM_BYTES_PER_LAUNCH = 2_043_648   # profiles/r1_scan_dpx_full.md (2.04 MB read + 0 written per launch)
+ALGO_INSTR_PER_CELL = 0.75          # one-pass scan: 1 add-max-relu per 2 cells + 1 three-input max per 4 cells
+ALGO_INSTR_PER_CELL_PASS1 = 0.375   # two-pass scan, pass 1: 1 add-max-relu per 4 cells + 1 three-input max per 8 cells
 ALU_LANES_PER_CLK_SM = 64           # integer/DPX pipe: 16 lanes/clk per SM sub-partition x 4 (guide + measured)
+ISSUE_LANES_PER_CLK_SM = 128        # one warp instruction per clock per SM sub-partition
+SMEM_BYTES_PER_CLK_SM = 128         # shared-memory data pipe: one 128-byte wavefront per clock per SM
+# ncu --set full captures of the dominant kernels at ONE launch size (config 2, 4096 reads); quoted only for that launch
+NCU_CAPTURES = {
+    "scan_filter_lq_kernel": {"dram_bytes": 2_074_624, "instr_per_cell": 0.848, "smem_bytes_per_cell": 0.5,
+                              "source": "profiles/r2_scan_filter_lq_full.md"},
+    "scan_filter_kernel": {"dram_bytes": 2_019_072, "instr_per_cell": 0.871, "smem_bytes_per_cell": 1.0,
+                           "source": "profiles/r1_scan_filter_full.md"},
+    "scan_dpx_kernel": {"dram_bytes": 2_043_648, "instr_per_cell": 1.54, "smem_bytes_per_cell": 2.0,
+                        "source": "profiles/r1_scan_dpx_full.md"},
+}
 
 
 class ClockSampler(threading.Thread):
@@ -133,63 +142,35 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); the metric is quoted on 2")
-    ap.add_argument("--reads", type=int, default=None, help="reads per step per GPU (default: the config's own count)")
-    ap.add_argument("--variant", type=int, default=0, help="scan kernel variant (0 = automatic)")
-    ap.add_argument("--read-len", type=int, default=None,
-                    help="diagnostic: keep only the config's read groups of this length (config 3's sweep, one length at a time)")
-    ap.add_argument("--mode", default="plain", choices=["plain", "fast", "pssm"],
-                    help="diagnostic: time the next-row scans (MaxSSmap_fast / base-quality PSSM) instead of the plain scan")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-nw", action="store_true", help="time the MaxSS stage only (diagnostic; not a bench value)")
-    ap.add_argument("--ref-reads-per-core", type=int, default=2)
-    ap.add_argument("--cigar-stride", type=int, default=16)
-    args = ap.parse_args()
-    cfg = gen.config(args.config)
-    if args.impl == "reference":
-        run_reference(args, cfg)
-        return
+def free_port() -> int:
+    import socket
+    sk = socket.socket()
+    sk.bind(("127.0.0.1", 0))
+    port = sk.getsockname()[1]
+    sk.close()
+    return port
 
-    import torch
-    import paper_1403_2136_b200 as mss
-    if not os.path.exists(mss.lib_path()) and int(os.environ.get("LOCAL_RANK", "0")) == 0:
-        from paper_1403_2136_b200 import build as mss_build      # in-tree build of libmss.so (nvcc, sm_100a); no fallback exists
-        mss_build.build()
-    for _ in range(600):                                         # other local ranks wait for rank 0's build
-        if os.path.exists(mss.lib_path()):
-            break
-        time.sleep(0.5)
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    dev = torch.device("cuda", local)
+def respawn_under_torchrun(args) -> None:
+    """`python bench.py --gpus N` (N > 1) with no launcher around it: start the N ranks ourselves, exactly as the driver
+    would (one process per GPU, torch.distributed.run, rendezvous on 127.0.0.1), and hand back their exit code."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
-    # ---- inputs: genome replicated, reads sharded by rank (independent units, no data-path collective) ------------
-    genome, _ = cfg.genome()
+
+def rank_inputs(cfg, args, rank: int, world: int, genome):
+    """This rank's batch of reads: the config's own reads on one GPU; with several ranks (weak scaling) or with --reads /
+    --read-len every rank draws its own batch from the same recipe, the seed offset by the rank."""
     groups = [g for g in cfg.groups if args.read_len in (None, g[1])]
     if not groups:
         raise SystemExit(f"config {cfg.c} has no read group of length {args.read_len}")
     m = max(g[1] for g in groups)
     n_reads = args.reads or sum(g[0] for g in groups)
-    if args.reads is None and args.read_len is None:
-        r = cfg.reads(genome) if world == 1 else None
-    else:
-        r = None
-    if r is None:   # ranks draw their own batch (weak scaling): same recipe, seed offset by rank
+    r = None
+    if args.reads is None and args.read_len is None and world == 1:
+        r = cfg.reads(genome)
+    if r is None:
         outs = []
         per = max(1, n_reads // len(groups))
         for gi, (_, mm, rate) in enumerate(groups):
@@ -199,7 +180,81 @@ def main():
                 pad = np.full((per, m), gen.N, dtype=np.uint8); pad[:, :mm] = o["reads"]; o["reads"] = pad
             outs.append(o)
         r = {k: np.concatenate([o[k] for o in outs]) for k in outs[0]}
-    reads, lens = r["reads"], r["lens"]
+    reads, lens = r["reads"].copy(), r["lens"]
+    n_with_n = 0
+    if args.n_frac > 0:                # real reads carry N calls (the profile has an N row): one N in a fraction of the reads
+        rng = np.random.Generator(np.random.PCG64(cfg.reads_seed + 31 + 7919 * rank))
+        pick = np.where(rng.random(reads.shape[0]) < args.n_frac)[0]
+        reads[pick, rng.integers(0, np.maximum(lens[pick], 1))] = gen.N
+        n_with_n = int(pick.size)
+    return reads, lens, m, n_with_n
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5; 6 = whole-genome-sized); the metric is quoted on 2")
+    ap.add_argument("--reads", type=int, default=None, help="reads per step per GPU (default: the config's own count)")
+    ap.add_argument("--variant", type=int, default=0, help="scan kernel variant (0 = automatic)")
+    ap.add_argument("--read-len", type=int, default=None,
+                    help="diagnostic: keep only the config's read groups of this length (config 3's sweep, one length at a time)")
+    ap.add_argument("--mode", default="plain", choices=["plain", "fast", "pssm"],
+                    help="diagnostic: time the next-row scans (MaxSSmap_fast / base-quality PSSM) instead of the plain scan")
+    ap.add_argument("--n-frac", type=float, default=0.0, help="diagnostic: fraction of reads that get one N (they take the unfiltered path)")
+    ap.add_argument("--query-sets", type=int, default=0, help="pass 1: 32-query sets per block (1, 2, 4; 0 = default) -- config 5's reads-per-block sweep")
+    ap.add_argument("--tile", type=int, default=0, help="pass 1: window starts per tile (0 = automatic)")
+    ap.add_argument("--arith", type=int, default=-1, help="pass 1 arithmetic: 0 int16 DPX, 1 fp16, 2 e5m2 bytes, -1 automatic")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-nw", action="store_true", help="time the MaxSS stage only (diagnostic; not a bench value)")
+    ap.add_argument("--ref-reads-per-core", type=int, default=2)
+    ap.add_argument("--cigar-stride", type=int, default=16)
+    ap.add_argument("--plumbing-only", action="store_true",
+                    help="test hook: run the launch / sharding / max-over-ranks / rank-0-print path on the CPU (gloo) with the "
+                         "device work replaced by a sleep; prints no metric value")
+    args = ap.parse_args()
+    cfg = gen.config(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        respawn_under_torchrun(args)
+
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != max(1, args.gpus) and rank == 0:
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} but the launcher started {world} rank(s); reporting n_gpus={world}\n")
+
+    if args.plumbing_only:
+        plumbing_only(args, cfg, rank, world)
+        return
+
+    import paper_1403_2136_b200 as mss
+    if not os.path.exists(mss.lib_path()) and local == 0:
+        from paper_1403_2136_b200 import build as mss_build      # in-tree build of libmss.so (nvcc, sm_100a); no fallback exists
+        mss_build.build()
+    for _ in range(600):                                         # other local ranks wait for rank 0's build
+        if os.path.exists(mss.lib_path()):
+            break
+        time.sleep(0.5)
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    from paper_1403_2136_b200.shard import max_over_ranks
+
+    # ---- inputs: genome replicated, reads sharded by rank (independent units, no data-path collective) ------------
+    genome, _ = cfg.genome()
+    reads, lens, m, n_with_n = rank_inputs(cfg, args, rank, world, genome)
     n_reads = reads.shape[0]
     packed, nmask = gen.pack_2bit(genome)
     rp, rn = gen.pack_reads(reads, lens)
@@ -217,16 +272,18 @@ def main():
     d_reads, d_mask, d_lens = h_reads.to(dev), h_mask.to(dev), h_lens.to(dev)
     sc = mss.Scoring()
     mss.mss_set_scan_variant(args.variant)
+    mss.mss_set_pass1_geometry(args.query_sets, args.tile, args.arith)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)          # > 126 MB L2
     stream = torch.cuda.current_stream()
     scored = lens.astype(np.float64) if args.mode != "fast" else np.ceil(lens.astype(np.float64) / 2)   # fast: every other base
-    cells_step = float(np.sum(scored)) * G.n_frag * cfg.frag_len * (2 if cfg.strands == 3 else 1)
+    ns = 2 if cfg.strands == 3 else 1
+    cells_step = float(np.sum(scored)) * G.n_frag * cfg.frag_len * ns
     d_qual, pssm_scale = None, 16
     if args.mode == "pssm":
         d_qual = torch.from_numpy(gen.make_quals(n_reads, m, cfg.reads_seed + 5)).to(dev)
 
     def step():
-        """resident inputs -> top-2 records -> NW score/pos/CIGAR, all on the device; returns (scan_ms event pair)."""
+        """resident inputs -> top-2 records -> NW score/pos/CIGAR, all on the device; returns the event triple."""
         e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         e0.record(stream)
         if args.mode == "fast":
@@ -261,9 +318,7 @@ def main():
     sampler.start()
     time.sleep(0.3)
     evs = []
-    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
-    step_ms = []
     mss.mss_set_pass_timing(True)
     pass_ms = []
     for _ in range(args.steps):
@@ -276,12 +331,9 @@ def main():
     scan_ms = [a.elapsed_time(b) for a, b, _ in evs]
     nw_ms = [b.elapsed_time(c) for _, b, c in evs]
     step_ms = [a.elapsed_time(c) for a, _, c in evs]
-    total_ms = sum(step_ms)                 # device time of exactly K steps (the flush writes are outside the events)
+    own_ms = sum(step_ms)                   # device time of exactly K steps (the flush writes are outside the events)
     clocks = sampler.stop()
-    if dist is not None:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(own_ms, dev)
     ms_per_step = total_ms / args.steps
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region ----------------------------------------
@@ -295,11 +347,7 @@ def main():
             t0 = time.perf_counter()
             out = mss.mss_map_align_host(G, h_reads, h_mask, h_lens, m, sc, cfg.strands, 30, args.cigar_stride, out=out)
             e2e_times.append(time.perf_counter() - t0)
-        e2e_s = sum(e2e_times) / len(e2e_times)
-        if dist is not None:
-            t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = max_over_ranks(sum(e2e_times) / len(e2e_times), dev)
         h2d = h_reads.numel() * 4 + h_mask.numel() * 4 + h_lens.numel() * 4
         d2h = sum(v.numel() * v.element_size() for v in out.values())
         same = bool((out["top2"] == top2.cpu()).all())
@@ -315,36 +363,59 @@ def main():
     peaks = measured_peaks()
     sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
-    peak_instr = n_sm * ALU_LANES_PER_CLK_SM * sm_max * 1e6              # thread-instr/s, ALU/DPX pipe at max clock
+    clk = sm_max * 1e6
+    peak_instr = n_sm * ALU_LANES_PER_CLK_SM * clk                        # thread-instr/s, ALU/DPX pipe at max clock
     scan_avg_ms = sum(scan_ms) / len(scan_ms)
     probe_rate, _ = mss.mss_probe_dpx_peak(2048)
     peak_source = f"{n_sm} SMs x {ALU_LANES_PER_CLK_SM} lanes/clk x {sm_max:.0f} MHz (clocks.max.sm of MEASURED_PEAKS.json)"
     p1_ms = sum(a for a, _ in pass_ms) / len(pass_ms)
     p2_ms = sum(b for _, b in pass_ms) / len(pass_ms)
-    if launch_info["variant"] == 7 and p1_ms > 0:
-        # two-pass scan: the dominant kernel is pass 1 (scan_filter_kernel), which touches every cell of the step
-        achieved = cells_step * ALGO_INSTR_PER_CELL_PASS1 / (p1_ms * 1e-3)
-        roofline = {"bound": "alu", "kernel": "scan_filter_kernel (pass 1 of the two-pass scan)", "achieved": achieved / 1e12,
-                    "peak": peak_instr / 1e12, "unit": "T thread-instr/s", "frac": achieved / peak_instr,
-                    "traffic": NCU_DRAM_BYTES_PASS1,
-                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1_scan_filter_full.md (ncu --set full, "
-                                      "one 4096-read launch: genome once, then L2; the 16-bit bounds written once)",
-                    "peak_source": peak_source, "algorithmic_instr_per_cell": ALGO_INSTR_PER_CELL_PASS1,
-                    "cells_per_launch": cells_step, "kernel_ms": p1_ms, "pass2_ms": p2_ms,
-                    "kernel_share_of_step": p1_ms / (ms_per_step if world == 1 else sum(step_ms) / len(step_ms)),
-                    "probe_dpx_peak": probe_rate / 1e12, "frac_of_probe": achieved / probe_rate if probe_rate > 0 else None,
-                    "whole_scan_vs_one_pass_floor": cells_step * ALGO_INSTR_PER_CELL / (scan_avg_ms * 1e-3) / peak_instr,
-                    "note": "whole_scan_vs_one_pass_floor counts 0.75 instr/cell, the floor of the exact one-pass formulation; the "
-                            "two-pass scan composes two Kadane steps per DPX instruction, so that figure may exceed 1"}
+    two_pass = launch_info["variant"] == 7 and p1_ms > 0
+    genome_bytes = cfg.genome_len * 3 / 8                                   # 2-bit words + N mask
+    l2_resident = genome_bytes < 100e6
+    n_chunks = max(1, launch_info["launches"] // 2) if two_pass else 1
+    if two_pass:
+        # the dominant kernel is pass 1, which touches every cell of the step
+        kernel = "scan_filter_lq_kernel" if launch_info["pass1_kernel"] >= 2 else "scan_filter_kernel"
+        kname = f"{kernel} (pass 1 of the two-pass scan)"
+        kernel_ms, algo = p1_ms, ALGO_INSTR_PER_CELL_PASS1
+        # DRAM bytes the launch has to move: the genome once per chunk of reads while it fits L2 (else once per resident wave
+        # of blocks: not modelled, null), the reads once, the 16-bit bounds written by pass 1 (and read back by pass 2)
+        bounds_bytes = n_reads * ns * G.n_frag * 2
+        traffic_model = (genome_bytes * n_chunks + h_reads.numel() * 4 + bounds_bytes) if l2_resident else None
     else:
-        achieved = cells_step * ALGO_INSTR_PER_CELL / (scan_avg_ms * 1e-3)
-        roofline = {"bound": "alu", "kernel": "scan_dpx_kernel", "achieved": achieved / 1e12, "peak": peak_instr / 1e12,
-                    "unit": "T thread-instr/s", "frac": achieved / peak_instr, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
-                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1_scan_dpx_full.md (ncu --set full, one "
-                                      "4096-read launch of this kernel: the 1.7 MB genome once, then L2)",
-                    "peak_source": peak_source, "algorithmic_instr_per_cell": ALGO_INSTR_PER_CELL, "cells_per_launch": cells_step,
-                    "kernel_ms": scan_avg_ms, "probe_dpx_peak": probe_rate / 1e12,
-                    "frac_of_probe": achieved / probe_rate if probe_rate > 0 else None}
+        kernel = "scan_dpx_kernel"
+        kname, kernel_ms, algo = kernel, scan_avg_ms, ALGO_INSTR_PER_CELL
+        traffic_model = (genome_bytes + h_reads.numel() * 4) if l2_resident else None
+    cap = NCU_CAPTURES[kernel]
+    cells_per_clk_sm = cells_step / (kernel_ms * 1e-3) / n_sm / clk
+    achieved = cells_step * algo / (kernel_ms * 1e-3)
+    same_launch_as_capture = (args.config == 2 and n_reads == 4096 and args.mode == "plain" and m == 100)
+    roofline = {
+        "bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T thread-instr/s",
+        "frac": achieved / peak_instr,
+        # ncu DRAM bytes are quoted only for the launch that was captured (config 2, 4096 reads); other launches get the model
+        "traffic": cap["dram_bytes"] if same_launch_as_capture else None, "traffic_source": cap["source"],
+        "traffic_model_bytes": traffic_model,
+        "traffic_model": "genome (2-bit + N mask) once per chunk of reads + packed reads + 16-bit pass-1 bounds; the genome stays in L2"
+                         if l2_resident else "genome larger than L2: streamed from HBM once per wave of blocks, not modelled",
+        "peak_source": peak_source, "algorithmic_instr_per_cell": algo, "cells_per_launch": cells_step / n_chunks,
+        "launches_per_step": n_chunks, "kernel_ms": kernel_ms, "pass2_ms": p2_ms if two_pass else None,
+        "kernel_share_of_step": kernel_ms / (sum(step_ms) / len(step_ms)),
+        "cells_per_clk_sm": cells_per_clk_sm,
+        "probe_dpx_peak": probe_rate / 1e12, "frac_of_probe": achieved / probe_rate if probe_rate > 0 else None,
+        # SURVEY 8(d) fraction (B): the whole scan against the exact one-pass floor of 0.75 instr/cell (may exceed 1: pass 1
+        # composes two Kadane steps per instruction and pass 2 restores exactness on ~1 % of the fragments)
+        "frac_survey_B": cells_step * ALGO_INSTR_PER_CELL / (scan_avg_ms * 1e-3) / peak_instr,
+        # what actually limits the kernel (ncu, profiles/): instructions issued per cell against one warp instruction per
+        # clock per sub-partition, and operand bytes per cell against the 128 B/clk/SM shared-memory pipe
+        "issue_frac": cells_per_clk_sm * cap["instr_per_cell"] / ISSUE_LANES_PER_CLK_SM,
+        "smem_frac": cells_per_clk_sm * cap["smem_bytes_per_cell"] / SMEM_BYTES_PER_CLK_SM,
+        "instr_per_cell_profiled": cap["instr_per_cell"], "smem_bytes_per_cell": cap["smem_bytes_per_cell"],
+        "limiter": ("issue slots + ALU pipe (PRMT widening and the 3-input max); shared memory at about half its rate"
+                    if kernel == "scan_filter_lq_kernel" else "shared-memory wavefronts"),
+        "limiter_source": cap["source"],
+    }
     line = {
         "metric": "MaxSS GCUPS (scan+top-2+NW step)", "value": cells_step * world / (ms_per_step * 1e-3) / 1e9,
         "unit": "GCUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
@@ -352,10 +423,12 @@ def main():
         "data": "synthetic",
         "config": {"workload": f"config {cfg.c} ({cfg.name}): {n_reads} reads x {m} bp per GPU vs {cfg.genome_len} bp genome, "
                                f"F={cfg.frag_len}, overlap={'m-1' if cfg.overlap < 0 else cfg.overlap}, both strands, top-2 + NW"
-                               + ("" if args.mode == "plain" else f" [diagnostic mode: {args.mode}]"),
+                               + ("" if args.mode == "plain" else f" [diagnostic mode: {args.mode}]")
+                               + ("" if not n_with_n else f" [diagnostic: {n_with_n} reads carry one N]"),
                    "reads_per_gpu": n_reads, "read_len": m, "genome_bp": cfg.genome_len, "frag_len": cfg.frag_len,
-                   "n_frag": G.n_frag, "l2": f"flushed between steps (256 MiB write); packed genome + N mask = {cfg.genome_len * 3 / 8 / 1e6:.1f} MB "
-                         + ("(L2-resident by design within a step)" if cfg.genome_len * 3 / 8 < 100e6 else "(streams from HBM)"),
+                   "n_frag": G.n_frag, "reads_with_n": n_with_n,
+                   "l2": f"flushed between steps (256 MiB write); packed genome + N mask = {genome_bytes / 1e6:.1f} MB "
+                         + ("(L2-resident by design within a step)" if l2_resident else "(streams from HBM)"),
                    "parallelism": f"reads sharded over {world} GPU(s), genome replicated, no collective",
                    "launch": launch_info},
         "reads_per_s": n_reads * world / (ms_per_step * 1e-3),
@@ -369,6 +442,41 @@ def main():
         line["cpu_baseline"] = cpu_baseline(cfg, genome, reads, lens)
     print(json.dumps(line), flush=True)
     if dist is not None:
+        dist.destroy_process_group()
+
+
+def plumbing_only(args, cfg, rank: int, world: int) -> None:
+    """The N > 1 host path of main() without a GPU: gloo process group, per-rank inputs, barrier, K "steps" whose device
+    time is a rank-dependent sleep, max over ranks, rank 0 prints one JSON line.  Used by tests/test_bench_launch.py."""
+    import hashlib
+    import torch
+    import torch.distributed as dist
+    from paper_1403_2136_b200.shard import max_over_ranks
+    if world > 1:
+        dist.init_process_group("gloo")
+    genome = gen.make_genome(20_000, cfg.genome_seed)[0]
+    args.reads = args.reads or 64
+    reads, lens, m, _ = rank_inputs(cfg, args, rank, world, genome)
+    digest = hashlib.sha256(reads.tobytes()).hexdigest()[:16]
+    if world > 1:
+        dist.barrier()
+    own_ms = 0.0
+    for _ in range(args.steps):
+        t0 = time.perf_counter()
+        time.sleep(0.005 * (rank + 1))
+        own_ms += 1e3 * (time.perf_counter() - t0)
+    if world > 1:
+        dist.barrier()
+    total_ms = max_over_ranks(own_ms)
+    digests = [digest]
+    if world > 1:
+        digests = [None] * world
+        dist.all_gather_object(digests, digest)
+    if rank == 0:
+        print(json.dumps({"plumbing_only": True, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                          "ms_per_step": total_ms / args.steps, "own_ms_rank0": own_ms, "reads_per_gpu": int(reads.shape[0]),
+                          "read_digests": digests, "scaling": "weak"}), flush=True)
+    if world > 1:
         dist.destroy_process_group()
 
 

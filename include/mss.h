@@ -248,7 +248,10 @@ int mss_version(void);                         /* 100*major + minor */
  * pass-1 block) is thread-local: it affects only calls made later on the same host thread.
  */
 int mss_set_scan_variant(int variant);
-typedef struct { int32_t variant, grid, block, smem_bytes, reads_per_block, tile_diagonals, launches; } mss_launch_info_t;
+typedef struct {
+    int32_t variant, grid, block, smem_bytes, reads_per_block, tile_diagonals, launches;
+    int32_t pass1_kernel;   /* two-pass scan: 1 = tile kernel, 2 / 3 / 4 = lane-per-query kernel with int16 DPX / fp16 / e5m2 operands; else 0 */
+} mss_launch_info_t;
 int mss_get_last_launch(mss_launch_info_t *out);
 
 /*
@@ -262,7 +265,7 @@ int mss_set_pass_timing(int on);
  * queries follow it.  Results do not depend on it; tests set it small to exercise the chunk loop. */
 int mss_set_two_pass_chunk_bytes(int64_t bytes);
 /* Geometry of the lane-per-query pass-1 kernel (this thread only; results do not depend on it).  query_sets: 32-query
- * sets per block, 1, 2 or 4 (reads per block = 16, 32 or 64 with both strands, twice that with one; 0 = default 1) --
+ * sets per block, 1, 2 or 4 (reads per block = 16, 32 or 64 with both strands, twice that with one; 0 = by batch size) --
  * BASELINE.json config 5's "reads-per-block swept".  tile_window_starts: window starts per tile (even; 0 = automatic:
  * the tile with the least padding of the fragment length that leaves room for two blocks per SM); a value no tile can
  * take makes pass 1 fall back to the tile kernel.  arithmetic: how the chains are computed -- 0 = packed int16 DPX

@@ -26,7 +26,7 @@ class _Scoring(C.Structure):
 
 class _LaunchInfo(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("variant", "grid", "block", "smem_bytes", "reads_per_block", "tile_diagonals",
-                                         "launches")]
+                                         "launches", "pass1_kernel")]
 
 
 @dataclass(frozen=True)

@@ -6,7 +6,7 @@
 namespace {
 thread_local int t_last_cuda = 0;
 thread_local int t_variant = 0;
-thread_local mss_launch_info_t t_info = { 0, 0, 0, 0, 0, 0, 0 };
+thread_local mss_launch_info_t t_info = { 0, 0, 0, 0, 0, 0, 0, 0 };
 
 int cuda_fail(cudaError_t e) { t_last_cuda = (int)e; return MSS_ERR_CUDA; }
 
@@ -161,7 +161,7 @@ int mss_map_reads_bounds(const mss_genome_t* g, const uint32_t* d_reads, const u
     p.istep = every_other ? 2 : 1; p.pssm = nullptr; p.pssm_stride = 0; p.ubound = nullptr; p.delta = 0;
     if (!scan_filter_supported(g, p)) return MSS_ERR_RANGE;
     if (h_delta) *h_delta = scan_filter_delta(p);
-    cudaError_t e = launch_scan_filter(g, p, d_bounds, (cudaStream_t)stream, nullptr, nullptr, nullptr, nullptr);
+    cudaError_t e = launch_scan_filter(g, p, d_bounds, (cudaStream_t)stream, nullptr, nullptr, nullptr, nullptr, nullptr);
     if (e != cudaSuccess) return cuda_fail(e);
     return MSS_OK;
 }

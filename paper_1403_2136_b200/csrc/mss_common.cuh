@@ -115,12 +115,12 @@ bool scan_filter_supported(const mss_genome* g, const ScanParams& p);
 int32_t scan_filter_delta(const ScanParams& p);
 void scan_filter_force_variant(int v, bool tile_kernel);
 cudaError_t launch_scan_filter(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
-                               int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out);
+                               int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out, int32_t* kind_out);
 // pass 1 in the lane-per-query layout (scan_filter_lq.cu): reads of up to 512 scored positions
 bool scan_filter_lq_supported(const mss_genome* g, const ScanParams& p);
 void scan_filter_lq_tune(int qsets, int half, int mode);
 cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
-                                  int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out);
+                                  int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out, int32_t* kind_out);
 size_t scan_two_pass_workspace(const mss_genome* g, int32_t n_reads, int32_t strands);
 cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p, void* ws, size_t ws_bytes,
                                  mss_top2_t* d_out, cudaStream_t st, mss_launch_info_t* info);

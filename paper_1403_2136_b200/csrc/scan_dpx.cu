@@ -361,7 +361,7 @@ cudaError_t launch_variant2(const mss_genome* g, const ScanParams& p, const DpxU
     scan_dpx_kernel<K, T, PSSM><<<(unsigned)blocks, T, smem, st>>>(p, ug, MP, ROWW, partial);
     if (info) {
         info->variant = id; info->grid = (int32_t)blocks; info->block = T; info->smem_bytes = (int32_t)smem;
-        info->reads_per_block = ug.reads_per_group; info->tile_diagonals = C::D; info->launches = 2;
+        info->reads_per_block = ug.reads_per_group; info->tile_diagonals = C::D; info->launches = 2; info->pass1_kernel = 0;
     }
     return cudaGetLastError();
 }
@@ -487,10 +487,16 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
 {
     (void)ws_bytes;
     const int32_t ns = p0.strands == 3 ? 2 : 1;
-    const int32_t chunk = two_pass_chunk(g, p0.n_reads, p0.strands);
+    // chunks of equal size (whole 64-read blocks) rather than full chunks and a small rest: every launch then fills the GPU
+    int32_t chunk = two_pass_chunk(g, p0.n_reads, p0.strands);
+    if (chunk < p0.n_reads) {
+        const int32_t n_chunks = (p0.n_reads + chunk - 1) / chunk;
+        int32_t even = ((p0.n_reads + n_chunks - 1) / n_chunks + 63) & ~63;
+        if (even < chunk) chunk = even;
+    }
     uint16_t* ubound = (uint16_t*)ws;
     int launches = 0;
-    int32_t fgrid = 0, fsmem = 0, ftile = 0, frpb = 0;
+    int32_t fgrid = 0, fsmem = 0, ftile = 0, frpb = 0, fkind = 0;
     t_events_used = 0;
     for (int32_t c0 = 0; c0 < p0.n_reads; c0 += chunk) {
         cudaEvent_t ev0 = nullptr, ev1 = nullptr, ev2 = nullptr;
@@ -506,7 +512,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
         p.reads_nmask = p0.reads_nmask ? p0.reads_nmask + (int64_t)c0 * ((p0.stride_words + 1) / 2) : nullptr;
         p.lens = p0.lens + c0;
         p.ubound = nullptr;
-        e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile, &frpb);
+        e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile, &frpb, &fkind);
         if (e != cudaSuccess) return e;
         if (ev1 && (e = cudaEventRecord(ev1, st)) != cudaSuccess) { t_events_used = 0; return e; }
         // pass 2: one read per block, every fragment range in one block (the bounds row decides what is scanned)
@@ -527,7 +533,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
     }
     if (info) {
         info->variant = 7; info->grid = fgrid; info->block = 0; info->smem_bytes = fsmem;
-        info->reads_per_block = frpb; info->tile_diagonals = ftile; info->launches = launches;
+        info->reads_per_block = frpb; info->tile_diagonals = ftile; info->launches = launches; info->pass1_kernel = fkind;
     }
     return cudaSuccess;
 }

@@ -272,10 +272,11 @@ int32_t scan_filter_delta(const ScanParams& p)
 }
 
 cudaError_t launch_scan_filter(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
-                               int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out)
+                               int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out, int32_t* kind_out)
 {
     if (!g_filter_tile_kernel && scan_filter_lq_supported(g, p))
-        return launch_scan_filter_lq(g, p, ubound, st, grid_out, smem_out, tile_out, rpb_out);
+        return launch_scan_filter_lq(g, p, ubound, st, grid_out, smem_out, tile_out, rpb_out, kind_out);
+    if (kind_out) *kind_out = 1;
     int v = pick_filter_variant(g, p);
     if (v < 0) return cudaErrorInvalidConfiguration;
     if (tile_out) *tile_out = 2 * kFVariants[v].K * kFVariants[v].T;

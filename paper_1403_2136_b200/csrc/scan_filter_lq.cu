@@ -34,17 +34,25 @@ namespace {
 
 constexpr int LQ_NW = 8;            // warps per block
 constexpr int LQ_K = 8;             // adjacent columns (chains) per thread and column group
-constexpr int LQ_NPL = 21;          // 16 dibase planes + 4 (c1, pad) planes + the all-zero plane of padding steps
+// planes of a tile: (c1, c2) -> c1*4 + c2; (c1, pad) -> 16 + c1 (last step of an odd-length query); 20 = all zero (padding
+// steps).  Blocks whose reads hold an N ("N" scores mismatch against everything, reading 6) add ten more:
+// (c1, N) -> 21 + c1, (N, c2) -> 25 + c2, (N, N) -> 29, (N, pad) -> 30, and take a smaller tile to make room for them.
+constexpr int LQ_NPL = 21;
+constexpr int LQ_NPL_N = 31;
 constexpr int LQ_ZERO_PLANE = 20;
 constexpr int LQ_MAX_QSETS = 4;
 enum { LQ_S16 = 0, LQ_F16 = 1, LQ_F8 = 2 };
 
-struct LqGeom {
-    int32_t n_groups, n_splits, frags_per_split, reads_per_group;
-    int32_t qsets;                  // query sets (of 32 lanes) per block: 1, 2 or 4; a set is scanned by NW / qsets warps
+struct LqTile {
     int32_t HALF, ROWW, NG;         // tile = 2*HALF window starts; plane stride (words); column groups per warp and tile
     int32_t COLS;                   // columns staged per tile (HALF + look-ahead)
     int32_t NRAW;                   // packed genome words a tile reads (even)
+};
+struct LqGeom {
+    int32_t n_groups, n_splits, frags_per_split, reads_per_group;
+    int32_t qsets;                  // query sets (of 32 lanes) per block: 1, 2 or 4; a set is scanned by NW / qsets warps
+    LqTile a;                       // blocks without an N in their reads: 21 planes
+    LqTile b;                       // blocks with one: 31 planes, smaller tile (HALF = 0: none fits, such reads stay unbounded)
 };
 
 __device__ __forceinline__ void lq_cp_async4(void* smem_dst, const void* gmem_src)
@@ -69,15 +77,10 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
     constexpr int K = LQ_K, NW = LQ_NW, T = 32 * NW;
     constexpr int NREG = PACKED ? NJ / 2 : NJ;
     extern __shared__ __align__(16) uint32_t smem[];
-    const int32_t ROWW = ug.ROWW, HALF = ug.HALF, D = 2 * ug.HALF;
-    uint32_t* planes = smem;                                    // LQ_NPL * ROWW
-    uint32_t* wres = planes + LQ_NPL * ROWW;                    // NW * 32: per (warp, lane) tile maximum
+    uint32_t* wres = smem;                                      // NW * 32: per (warp, lane) tile maximum
     int32_t* qnj = (int32_t*)(wres + NW * 32);                  // 32 * qsets: double steps of a query; 0 = not scanned
     int32_t* qm = qnj + 32 * LQ_MAX_QSETS;                      // 32 * qsets: read length
-    uint32_t* rawp = (uint32_t*)(qm + 32 * LQ_MAX_QSETS);       // 2 * NRAW: packed genome words of this tile / the next (cp.async)
-    uint32_t* rawn = rawp + 2 * ug.NRAW;                        // 2 * (NRAW / 2 + 1): N-mask words
-    const int32_t words_before = LQ_NPL * ROWW + NW * 32 + 2 * 32 * LQ_MAX_QSETS + 2 * ug.NRAW + 2 * (ug.NRAW / 2 + 1);
-    uint8_t* codes = reinterpret_cast<uint8_t*>(smem + ((words_before + 3) & ~3));   // 16 * NRAW one-hot base codes (16-byte aligned)
+    uint32_t* planes = (uint32_t*)(qm + 32 * LQ_MAX_QSETS);     // NPL * ROWW (the tile geometry is chosen below)
     uint8_t* sq = reinterpret_cast<uint8_t*>(planes);           // prologue only: strand-oriented base codes, row = query
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -91,10 +94,10 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
     const int32_t istep = p.istep;
     const int32_t wps = NW / ug.qsets;                          // warps per query set
     const int32_t set = warp / wps, ws = warp % wps;
-    const int32_t CW = HALF / wps;                              // columns of a tile scanned by one warp
     const int32_t sq_stride = (p.max_len + 3) & ~3;
 
     // ---- a1 read prep, step 1: strand-oriented base codes of every query of the block (bytes; 4 = N) -----------------
+    bool any_n = false;
     for (int32_t q = warp; q < 32 * ug.qsets; q += NW) {
         int32_t njq = 0, m = 0;
         if (q < nq) {
@@ -113,12 +116,23 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                 }
             }
             has_n = __any_sync(0xffffffffu, has_n);
+            any_n |= has_n;
             const int32_t steps = ok ? (m + istep - 1) / istep : 0;
-            njq = (ok && !has_n) ? (steps + 1) / 2 : 0;             // a query holding an N is not scanned: bound 0xFFFF
+            // not scanned (bound 0xFFFF): bad lengths, and reads with an N when no tile with the N planes fits
+            njq = (ok && !(has_n && ug.b.HALF == 0)) ? (steps + 1) / 2 : 0;
         }
         if (lane == 0) { qnj[q] = njq; qm[q] = m; }
     }
-    __syncthreads();
+    // ---- the block's tile: the large one, or the one with the N planes if any of its reads holds an N ----------------
+    const bool with_n = __syncthreads_or(any_n ? 1 : 0) != 0 && ug.b.HALF != 0;
+    const LqTile tg = with_n ? ug.b : ug.a;
+    const int32_t NPL = with_n ? LQ_NPL_N : LQ_NPL;
+    const int32_t ROWW = tg.ROWW, HALF = tg.HALF, D = 2 * tg.HALF;
+    const int32_t CW = HALF / wps;                              // columns of a tile scanned by one warp
+    uint32_t* rawp = planes + NPL * ROWW;                       // 2 * NRAW: packed genome words of this tile / the next (cp.async)
+    uint32_t* rawn = rawp + 2 * tg.NRAW;                        // 2 * (NRAW / 2 + 1): N-mask words
+    const int32_t words_before = NW * 32 + 2 * 32 * LQ_MAX_QSETS + NPL * ROWW + 2 * tg.NRAW + 2 * (tg.NRAW / 2 + 1);
+    uint8_t* codes = reinterpret_cast<uint8_t*>(smem + ((words_before + 3) & ~3));   // 16 * NRAW one-hot base codes (16-byte aligned)
 
     // ---- step 2: this lane's query -> plane offsets in registers -----------------------------------------------------
     // a column is a word (LQ_S16, LQ_F16) or half a word (LQ_F8: columns 2c, 2c+1 share word c; every offset below is even)
@@ -130,16 +144,18 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
         uint32_t plane = LQ_ZERO_PLANE, col = 0u;                   // padding step: adds 0
         if (j < mynj) {
             const int32_t i1 = 2 * j * istep, i2 = i1 + istep;
-            const uint32_t b1 = sq[myq * sq_stride + i1];
-            const uint32_t b2 = (i2 < mym) ? sq[myq * sq_stride + i2] : 4u;     // 4 = past the end: the (c1, pad) plane
-            plane = b1 * 5u + b2; col = (uint32_t)i1;
+            const uint32_t b1 = sq[myq * sq_stride + i1];                       // 0..3, 4 = N
+            const uint32_t b2 = (i2 < mym) ? sq[myq * sq_stride + i2] : 5u;     // 5 = past the end (pad)
+            if (b1 < 4u) plane = b2 < 4u ? b1 * 4u + b2 : (b2 == 5u ? 16u + b1 : 21u + b1);
+            else plane = b2 < 4u ? 25u + b2 : (b2 == 5u ? 30u : 29u);
+            col = (uint32_t)i1;
         }
         const uint32_t cw = col + (uint32_t)(ws * CW);              // column of chain 0, group 0
         const uint32_t w = plane * (uint32_t)ROWW + (MODE == LQ_F8 ? cw >> 1 : cw);
         if (PACKED) {
             if (j & 1) off[j >> 1] |= w << 16; else off[j >> 1] = w;
         } else {
-            asm("shl.b32 %0, %1, 2;" : "=r"(off[j]) : "r"(w));     // opaque: keeps ptxas from storing w and re-scaling it (LEA) per use
+            off[j] = w * 4u;
         }
     }
     // double steps this warp runs: the longest query of its set, rounded up to the pair the loop body handles
@@ -180,10 +196,10 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
         const int32_t f = f_begin + it / tiles_per_frag, tile = it % tiles_per_frag;
         const int64_t g0 = (int64_t)f * p.F + (int64_t)tile * D;
         const int64_t w0 = g0 >> 4;
-        uint32_t* rp = rawp + (it & 1) * ug.NRAW;
-        uint32_t* rn = rawn + (it & 1) * (ug.NRAW / 2 + 1);
-        for (int32_t i = tid; i < ug.NRAW; i += T) lq_cp_async4(rp + i, p.gpacked + w0 + i);
-        for (int32_t i = tid; i < ug.NRAW / 2 + 1; i += T) lq_cp_async4(rn + i, p.gnmask + (w0 >> 1) + i);
+        uint32_t* rp = rawp + (it & 1) * tg.NRAW;
+        uint32_t* rn = rawn + (it & 1) * (tg.NRAW / 2 + 1);
+        for (int32_t i = tid; i < tg.NRAW; i += T) lq_cp_async4(rp + i, p.gpacked + w0 + i);
+        for (int32_t i = tid; i < tg.NRAW / 2 + 1; i += T) lq_cp_async4(rn + i, p.gnmask + (w0 >> 1) + i);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     if (n_tiles > 0) prefetch(0);
@@ -201,10 +217,10 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
             fold();
             // ---- a2: raw words -> one byte per genome position: one-hot of the base (1, 2, 4, 8), 0 = N or not readable
             {
-                const uint32_t* rp = rawp + (it & 1) * ug.NRAW;
-                const uint32_t* rn = rawn + (it & 1) * (ug.NRAW / 2 + 1);
+                const uint32_t* rp = rawp + (it & 1) * tg.NRAW;
+                const uint32_t* rn = rawn + (it & 1) * (tg.NRAW / 2 + 1);
                 const int64_t w0 = g0 >> 4;
-                for (int32_t i = tid; i < ug.NRAW; i += T) {
+                for (int32_t i = tid; i < tg.NRAW; i += T) {
                     const uint32_t w = rp[i];
                     const int64_t W = w0 + i;
                     const uint32_t mk = (rn[(int32_t)((W >> 1) - (w0 >> 1))] >> (16u * (uint32_t)(W & 1))) & 0xFFFFu;
@@ -225,7 +241,7 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
             // ---- a2: codes -> dibase planes ----------------------------------------------------------------------
             const int32_t sh = (int32_t)(g0 & 15);                  // codes[sh + x] = genome position g0 + x
             if (MODE != LQ_F8) {
-                for (int32_t x = tid; x < ug.COLS; x += T) {
+                for (int32_t x = tid; x < tg.COLS; x += T) {
                     const uint32_t lo1 = codes[sh + x], lo2 = codes[sh + x + istep];
                     const uint32_t hi1 = codes[sh + x + HALF], hi2 = codes[sh + x + HALF + istep];
 #pragma unroll
@@ -235,11 +251,16 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                         for (uint32_t c2 = 0; c2 < 4; c2++) {
                             const uint32_t nl = ml + ((lo2 >> c2) & 1u), nh = mh + ((hi2 >> c2) & 1u);
                             const uint32_t vl = nl == 2 ? e2_2 : (nl == 1 ? e2_1 : e2_0), vh = nh == 2 ? e2_2 : (nh == 1 ? e2_1 : e2_0);
-                            planes[(c1 * 5 + c2) * ROWW + x] = vl | (vh << 16);
+                            planes[(c1 * 4 + c2) * ROWW + x] = vl | (vh << 16);
                         }
-                        planes[(c1 * 5 + 4) * ROWW + x] = (ml ? e1_1 : e1_0) | ((mh ? e1_1 : e1_0) << 16);
+                        planes[(16 + c1) * ROWW + x] = (ml ? e1_1 : e1_0) | ((mh ? e1_1 : e1_0) << 16);
+                        if (with_n) {                               // (c1, N): the second position never matches; (N, c): the first
+                            planes[(21 + c1) * ROWW + x] = (ml ? e2_1 : e2_0) | ((mh ? e2_1 : e2_0) << 16);
+                            planes[(25 + c1) * ROWW + x] = (((lo2 >> c1) & 1u) ? e2_1 : e2_0) | ((((hi2 >> c1) & 1u) ? e2_1 : e2_0) << 16);
+                        }
                     }
                     planes[LQ_ZERO_PLANE * ROWW + x] = 0u;
+                    if (with_n) { planes[29 * ROWW + x] = e2_0 | (e2_0 << 16); planes[30 * ROWW + x] = e1_0 | (e1_0 << 16); }
                 }
             } else {
                 // word xw = columns 2xw, 2xw + 1, bytes (lo, hi, lo', hi').  The four lanes' one-hot codes go into the four
@@ -248,7 +269,7 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                 // count to its operand byte: 3 instructions per plane word
                 const uint32_t tab2 = (e2_0 >> 8) | (e2_1 & 0xFF00u) | ((e2_2 & 0xFF00u) << 8);
                 const uint32_t tab1 = (e1_0 >> 8) | (e1_1 & 0xFF00u);
-                for (int32_t xw = tid; xw < ug.COLS / 2; xw += T) {
+                for (int32_t xw = tid; xw < tg.COLS / 2; xw += T) {
                     const uint8_t* c0 = codes + sh + 2 * xw;
                     const uint32_t oh1 = c0[0] | (c0[HALF] << 4) | (c0[1] << 8) | (c0[HALF + 1] << 12);
                     const uint32_t oh2 = c0[istep] | (c0[HALF + istep] << 4) | (c0[1 + istep] << 8) | (c0[HALF + 1 + istep] << 12);
@@ -259,24 +280,29 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                     for (uint32_t c1 = 0; c1 < 4; c1++) {
 #pragma unroll
                         for (uint32_t c2 = 0; c2 < 4; c2++)
-                            planes[(c1 * 5 + c2) * ROWW + xw] = __byte_perm(tab2, 0u, A[c1] + Bm[c2]);
-                        planes[(c1 * 5 + 4) * ROWW + xw] = __byte_perm(tab1, 0u, A[c1]);
+                            planes[(c1 * 4 + c2) * ROWW + xw] = __byte_perm(tab2, 0u, A[c1] + Bm[c2]);
+                        planes[(16 + c1) * ROWW + xw] = __byte_perm(tab1, 0u, A[c1]);
+                        if (with_n) {                               // (c1, N): the second position never matches; (N, c): the first
+                            planes[(21 + c1) * ROWW + xw] = __byte_perm(tab2, 0u, A[c1]);
+                            planes[(25 + c1) * ROWW + xw] = __byte_perm(tab2, 0u, Bm[c1]);
+                        }
                     }
                     planes[LQ_ZERO_PLANE * ROWW + xw] = 0u;
+                    if (with_n) { planes[29 * ROWW + xw] = (e2_0 >> 8) * 0x01010101u; planes[30 * ROWW + xw] = (e1_0 >> 8) * 0x01010101u; }
                 }
             }
             __syncthreads();
 
             // ---- a3: this lane's query against the warp's columns of the tile --------------------------------------
             uint32_t tmax = 0u;
-            for (int32_t g = 0; g < ug.NG; g++) {
+            for (int32_t g = 0; g < tg.NG; g++) {
                 const char* pg = planes_b + g * (MODE == LQ_F8 ? K * 2 : K * 4);    // warp-uniform group base
                 uint32_t H[K], B[K];
 #pragma unroll
                 for (int k = 0; k < K; k++) { H[k] = 0u; B[k] = 0u; }
 #pragma unroll
                 for (int j = 0; j < NJ; j += 2) {
-                    if (j >= njb) break;
+                    if ((j & 7) == 0 && j >= njb) break;            // padding steps add 0: the check only saves time, so it is coarse
                     uint32_t o0, o1;
                     if (PACKED) {                                   // volatile: unpacked per use, or the compiler hoists all NJ results out of the group loop and spills them
                         uint32_t lo, hi;
@@ -349,7 +375,7 @@ bool lq_e5m2_exact(int32_t v)
 }
 
 struct LqSmem { int32_t ROWW, COLS, NRAW; size_t bytes; };
-LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode)
+LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode, int npl)
 {
     // columns read: chain column < HALF, plus the column of the last double step (< max_len rounded up to even steps)
     LqSmem s;
@@ -361,13 +387,13 @@ LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode)
     // genome positions a tile reads: [g0, g0 + HALF + COLS + istep), from the 16-aligned position below g0
     s.NRAW = ((half + s.COLS + istep + 15 + 15) / 16 + 1) & ~1;
     // planes, wres, qnj + qm, raw words (2 buffers), raw mask words (2 buffers), pad to 16 bytes, codes
-    size_t words = (size_t)LQ_NPL * roww + LQ_NW * 32 + 2 * 32 * LQ_MAX_QSETS + 2 * s.NRAW + 2 * (s.NRAW / 2 + 1);
+    size_t words = (size_t)npl * roww + LQ_NW * 32 + 2 * 32 * LQ_MAX_QSETS + 2 * s.NRAW + 2 * (s.NRAW / 2 + 1);
     words = (words + 3) & ~(size_t)3;
     s.bytes = words * 4 + (size_t)16 * s.NRAW;
     return s;
 }
 
-thread_local int t_lq_qsets = 1;       // tuning hook: query sets per block (reads per block = 16 * qsets with both strands)
+thread_local int t_lq_qsets = 0;       // tuning hook: query sets per block (reads per block = 16 * qsets with both strands); 0 = by batch size
 thread_local int t_lq_half = 0;        // tuning hook: force the tile (0 = automatic)
 thread_local int t_lq_mode = -1;       // tuning hook: force the arithmetic (-1 = automatic)
 
@@ -385,29 +411,49 @@ int lq_mode(const ScanParams& p)
 
 // the tile: 2*HALF window starts, HALF a multiple of the columns one more group of every warp of a set adds;
 // least padding of the fragment length first, larger tiles on ties; two blocks per SM must fit
-bool lq_pick(const mss_genome* g, const ScanParams& p, int32_t qsets, int mode, LqGeom* out)
+bool lq_pick_tile(const mss_genome* g, const ScanParams& p, int32_t qsets, int mode, int npl, int32_t forced_half, LqTile* out, size_t* bytes)
 {
     const int32_t unit = (LQ_NW / qsets) * LQ_K;
     const size_t prologue = (size_t)32 * qsets * ((p.max_len + 3) & ~3);
     int32_t best = 0; double best_waste = 1e30;
     for (int32_t half = unit; half <= 4096; half += unit) {
-        if (t_lq_half > 0 && half != t_lq_half) continue;
+        if (forced_half > 0 && half != forced_half) continue;
         if (half < 128) continue;
-        LqSmem s = lq_smem(half, p.max_len, p.istep, mode);
+        LqSmem s = lq_smem(half, p.max_len, p.istep, mode, npl);
         if (s.bytes * 2 + 4096 > (size_t)g->max_smem_optin) break;
-        if ((size_t)LQ_NPL * s.ROWW * 4 < prologue) continue;      // the prologue borrows the plane area
-        if ((int64_t)LQ_NPL * s.ROWW + 4096 > 65535) break;          // packed 16-bit word offsets
+        if ((size_t)npl * s.ROWW * 4 < prologue) continue;         // the prologue borrows the plane area
+        if ((int64_t)npl * s.ROWW + 4096 > 65535) break;             // packed 16-bit word offsets
         int32_t D = 2 * half;
         double waste = (double)((g->frag_len + D - 1) / D) * D / g->frag_len;
         waste *= 1.0 + 0.02 * (double)(s.COLS - half) / half;       // look-ahead columns are staged, not scanned: mild preference for large tiles
         if (waste < best_waste - 1e-9) { best_waste = waste; best = half; }
     }
     if (!best) return false;
-    if (out) {
-        LqSmem s = lq_smem(best, p.max_len, p.istep, mode);
-        out->HALF = best; out->ROWW = s.ROWW; out->COLS = s.COLS; out->NRAW = s.NRAW; out->qsets = qsets; out->NG = best / unit;
-    }
+    LqSmem s = lq_smem(best, p.max_len, p.istep, mode, npl);
+    if (out) { out->HALF = best; out->ROWW = s.ROWW; out->COLS = s.COLS; out->NRAW = s.NRAW; out->NG = best / unit; }
+    if (bytes) *bytes = s.bytes;
     return true;
+}
+
+// both tiles of a launch: the one of N-free blocks decides whether the kernel applies at all
+bool lq_pick(const mss_genome* g, const ScanParams& p, int32_t qsets, int mode, LqGeom* out, size_t* bytes)
+{
+    LqTile a, b;
+    size_t ba = 0, bb = 0;
+    if (!lq_pick_tile(g, p, qsets, mode, LQ_NPL, t_lq_half, &a, &ba)) return false;
+    if (!lq_pick_tile(g, p, qsets, mode, LQ_NPL_N, 0, &b, &bb)) { b = LqTile{0, 0, 0, 0, 0}; bb = 0; }
+    if (out) { out->a = a; out->b = b; out->qsets = qsets; }
+    if (bytes) *bytes = ba > bb ? ba : bb;
+    return true;
+}
+
+// query sets per block: more sets amortise the tile staging over more queries (measured on config 2: 131.0 / 133.0 / 133.8
+// cells/clk/SM with 1 / 2 / 4 sets), fewer keep the grid fine for small batches
+int32_t lq_qsets(const ScanParams& p)
+{
+    if (t_lq_qsets) return t_lq_qsets;
+    const int64_t queries = (int64_t)p.n_reads * (p.strands == 3 ? 2 : 1);
+    return queries >= 65536 ? 4 : (queries >= 16384 ? 2 : 1);
 }
 
 int32_t lq_double_steps(const ScanParams& p)
@@ -438,7 +484,7 @@ cudaError_t lq_launch(int mode, const ScanParams& p, const LqGeom& ug, uint16_t*
 
 void scan_filter_lq_tune(int qsets, int half, int mode)
 {
-    t_lq_qsets = (qsets == 2 || qsets == 4) ? qsets : 1;
+    t_lq_qsets = (qsets == 1 || qsets == 2 || qsets == 4) ? qsets : 0;
     t_lq_half = half > 0 ? half : 0;
     t_lq_mode = (mode >= 0 && mode <= 2) ? mode : -1;
 }
@@ -446,15 +492,17 @@ void scan_filter_lq_tune(int qsets, int half, int mode)
 bool scan_filter_lq_supported(const mss_genome* g, const ScanParams& p)
 {
     if (lq_double_steps(p) > 128) return false;                 // longer queries: the tile kernel of scan_filter.cu
-    return lq_pick(g, p, t_lq_qsets, lq_mode(p), nullptr);
+    return lq_pick(g, p, lq_qsets(p), lq_mode(p), nullptr, nullptr);
 }
 
 cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
-                                  int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out)
+                                  int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out, int32_t* kind_out)
 {
     LqGeom ug;
     const int mode = lq_mode(p);
-    if (!lq_pick(g, p, t_lq_qsets, mode, &ug)) return cudaErrorInvalidConfiguration;
+    if (kind_out) *kind_out = 2 + mode;
+    size_t smem = 0;
+    if (!lq_pick(g, p, lq_qsets(p), mode, &ug, &smem)) return cudaErrorInvalidConfiguration;
     const int32_t ns = p.strands == 3 ? 2 : 1;
     ug.reads_per_group = 32 * ug.qsets / ns;
     ug.n_groups = (p.n_reads + ug.reads_per_group - 1) / ug.reads_per_group;
@@ -465,12 +513,19 @@ cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint
     if (want > g->n_frag) want = g->n_frag;
     ug.frags_per_split = (int32_t)((g->n_frag + want - 1) / want);
     ug.n_splits = (g->n_frag + ug.frags_per_split - 1) / ug.frags_per_split;
-    const size_t smem = lq_smem(ug.HALF, p.max_len, p.istep, mode).bytes;
     if (grid_out) *grid_out = (int32_t)((int64_t)ug.n_groups * ug.n_splits);
     if (smem_out) *smem_out = (int32_t)smem;
-    if (tile_out) *tile_out = 2 * ug.HALF;
+    if (tile_out) *tile_out = 2 * ug.a.HALF;
     if (rpb_out) *rpb_out = ug.reads_per_group;
     const int32_t nj = lq_double_steps(p);
+    // padding steps cost time (the early-exit check is coarse): the common read lengths get a tight instance of the
+    // fast arithmetic (36, 51, 76, 100 bp)
+    if (mode == LQ_F8) {
+        if (nj <= 18) return lq_launch3<18, false, LQ_F8>(p, ug, ubound, st, smem);
+        if (nj <= 26) return lq_launch3<26, false, LQ_F8>(p, ug, ubound, st, smem);
+        if (nj > 32 && nj <= 38) return lq_launch3<38, false, LQ_F8>(p, ug, ubound, st, smem);
+        if (nj > 38 && nj <= 50) return lq_launch3<50, false, LQ_F8>(p, ug, ubound, st, smem);
+    }
     if (nj <= 32) return lq_launch<32, false>(mode, p, ug, ubound, st, smem);
     if (nj <= 64) return lq_launch<64, false>(mode, p, ug, ubound, st, smem);
     if (nj <= 80) return lq_launch<80, false>(mode, p, ug, ubound, st, smem);

@@ -131,7 +131,7 @@ cudaError_t launch_scan_generic(const mss_genome* g, const ScanParams& p, void* 
     }
     if (info) {
         info->variant = 1; info->block = GEN_THREADS; info->smem_bytes = p.max_len + 16;
-        info->reads_per_block = 1; info->tile_diagonals = g->frag_len; info->launches = launches;
+        info->reads_per_block = 1; info->tile_diagonals = g->frag_len; info->launches = launches; info->pass1_kernel = 0;
     }
     return cudaGetLastError();
 }

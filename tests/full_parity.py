@@ -116,7 +116,10 @@ def main():
         if not ok:
             bad_nw.append(int(i))
     # the NW comparison assumes the GPU hit equals the oracle's hit, which the top-2 comparison establishes
-    cells = float(np.sum(lens if args.mode != "fast" else -(-lens // 2))) * G.n_frag * cfg.frag_len * (2 if cfg.strands == 3 else 1)
+    per_frag = G.n_frag * cfg.frag_len * (2 if cfg.strands == 3 else 1)
+    scored = lens if args.mode != "fast" else -(-lens // 2)
+    cells = float(np.sum(scored)) * per_frag                               # cells of the whole batch (what the GPU mapped)
+    cells_compared = float(np.sum(scored[args.skip:stop])) * per_frag      # cells of the slice the oracle re-computed
     summary = {
         "config": cfg.c, "name": cfg.name, "mode": args.mode, "reads": int(n), "read_len_max": int(m), "n_frag": int(G.n_frag),
         "cells": cells, "top2_compared": int(checked - args.skip), "first_read_compared": int(args.skip), "top2_mismatches": len(bad_top2), "first_bad_top2": bad_top2[:5],
@@ -124,7 +127,8 @@ def main():
         "ties_best_eq_second": int(np.sum(got[:, 0, 2] == got[:, 1, 2])),
         "ratio_ge_0.9": int(np.sum(10 * got[:, 1, 2].astype(np.int64) >= 9 * got[:, 0, 2].astype(np.int64))),
         "top1_within_1_of_truth": float(np.mean(np.abs(got[:, 0, 0] - r["start"] // cfg.frag_len) <= 1)),
-        "gpu_wall_s": gpu_s, "oracle_wall_s": cpu_s, "oracle_cores": cores, "oracle_gcups": cells / cpu_s / 1e9,
+        "gpu_wall_s": gpu_s, "oracle_wall_s": cpu_s, "oracle_cores": cores, "cells_compared": cells_compared,
+        "oracle_gcups": cells_compared / cpu_s / 1e9,
         "launch": info, "inputs_sha256": gen.sha256_of(genome, reads, lens),
     }
     line = json.dumps(summary)
