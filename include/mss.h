@@ -181,10 +181,12 @@ int mss_pssm_build(const uint8_t *d_qual, int32_t qual_stride, const int32_t *d_
 /*
  * mss_map_reads with s(read[i], genome base) replaced by the read's own table: pmatch_i if the bases are equal (and
  * neither is N) else pmismatch_i; on the reverse strand position i of the reverse-complemented read carries the
- * entry of original position len-1-i.  `bound` states the table's range for the 16-bit lane check:
- * bound.match >= every pmatch_i, bound.mismatch <= every pmismatch_i (for a table from mss_pssm_build:
- * {scale*match, scale*mismatch, scale*gap}); max_len*bound.match <= 32767 else MSS_ERR_RANGE; entries outside the
- * stated bound give undefined scores.  pssm_stride >= max_len.  Workspace: mss_map_workspace_bytes.
+ * entry of original position len-1-i.  `bound` states the table's range for the 16-bit lane check and for the slack
+ * of the two-pass scan's bounds (min(PM, -PMM) - PMM: a tight bound prunes better): bound.match >= every pmatch_i,
+ * bound.mismatch <= every pmismatch_i (for a table from mss_pssm_build: {scale*match, -ceil(scale*|mismatch|/3),
+ * scale*gap}); max_len*bound.match <= 32767 else MSS_ERR_RANGE; entries outside the stated bound give undefined
+ * scores.  pssm_stride >= max_len.  Workspace: mss_map_workspace_bytes.  The scan is the two-pass scan where the geometry
+ * allows it (pass 1: scan_filter_lq_kernel in its PSSM form), else the exact kernel on every fragment.
  */
 int mss_map_reads_pssm(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
                        int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
@@ -283,11 +285,18 @@ int mss_get_pass_times(float *h_pass1_ms, float *h_pass2_ms);
  * every_other != 0 bounds the MaxSSmap_fast scores instead.  MSS_ERR_RANGE if the geometry has no two-pass path
  * (fewer than 8 fragments, frag_len < 256, 2*match or 2*mismatch outside int16).  mss_map_reads itself uses these
  * bounds only to skip fragments that cannot reach a read's top-2; its records are those of the one-pass scan.
+ * Reads holding an N are bounded like any other by the lane-per-query kernel; the tile kernel marks them 0xFFFF.
+ * mss_map_reads_bounds_pssm: the same for base-quality scoring (table and `bound` as for mss_map_reads_pssm); *h_delta
+ * = min(bound.match, -bound.mismatch) - bound.mismatch.
  */
 int mss_map_reads_bounds(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
                          int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
                          mss_scoring_t sc, int32_t strands, int32_t every_other, void *stream,
                          uint16_t *d_bounds, int32_t *h_delta);
+int mss_map_reads_bounds_pssm(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
+                              int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
+                              const uint32_t *d_pssm, int32_t pssm_stride, mss_scoring_t bound, int32_t strands,
+                              void *stream, uint16_t *d_bounds, int32_t *h_delta);
 
 /*
  * Live measurement of the integer/DPX issue peak the scan's roofline is quoted against: runs `iters` dependent

@@ -86,6 +86,8 @@ def lib() -> C.CDLL:
     L.mss_get_pass_times.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]; L.mss_get_pass_times.restype = C.c_int
     L.mss_map_reads_bounds.argtypes = [vp, vp, vp, i32, vp, i32, i32, _Scoring, i32, i32, vp, vp, C.POINTER(i32)]
     L.mss_map_reads_bounds.restype = C.c_int
+    L.mss_map_reads_bounds_pssm.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, i32, _Scoring, i32, vp, vp, C.POINTER(i32)]
+    L.mss_map_reads_bounds_pssm.restype = C.c_int
     L.mss_map_reads_fast.argtypes = L.mss_map_reads.argtypes; L.mss_map_reads_fast.restype = C.c_int
     L.mss_pssm_build.argtypes = [vp, i32, vp, i32, _Scoring, i32, vp, vp, i32]; L.mss_pssm_build.restype = C.c_int
     L.mss_map_reads_pssm.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, i32, _Scoring, i32, vp, sz, vp, vp]
@@ -230,9 +232,25 @@ def mss_map_reads_bounds(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int
     return out, delta.value
 
 
+def mss_map_reads_bounds_pssm(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, d_pssm, bound: Scoring,
+                              strands: int = MSS_BOTH, stream=None):
+    """Pass 1 of the two-pass scan under base-quality scoring: -> (uint16 bounds as an int16 tensor, delta)."""
+    torch = _torch()
+    n = int(d_lens.numel())
+    ns = 2 if strands == MSS_BOTH else 1
+    out = torch.empty((n, ns, g.n_frag), dtype=torch.int16, device=d_lens.device)
+    delta = C.c_int32()
+    _check(lib().mss_map_reads_bounds_pssm(g.handle, _ptr(d_reads), _ptr(d_reads_nmask), int(d_reads.shape[1]), _ptr(d_lens), n,
+                                           max_len, _ptr(d_pssm), int(d_pssm.shape[1]), bound.c(), strands, _stream(stream),
+                                           _ptr(out), C.byref(delta)), "mss_map_reads_bounds_pssm")
+    return out, delta.value
+
+
 def pssm_bound(scoring: Scoring, scale: int) -> Scoring:
-    """The range of a table built by mss_pssm_build(scoring, scale): {scale*match, scale*mismatch, scale*gap}."""
-    return Scoring(scale * scoring.match, scale * scoring.mismatch, scale * scoring.gap)
+    """The range of a table built by mss_pssm_build(scoring, scale): pmatch <= scale*match, and pmismatch =
+    round(scale*mismatch*x/3) with x <= 1 >= -ceil(scale*|mismatch|/3); the gap is scale*gap.  The tight
+    mismatch bound matters: the slack of the two-pass scan's bounds is min(PM, -PMM) - PMM."""
+    return Scoring(scale * scoring.match, -((scale * -scoring.mismatch + 2) // 3), scale * scoring.gap)
 
 
 def mss_pssm_build(d_qual, d_lens, scoring: Scoring = Scoring(), scale: int = 16, pssm_stride: int | None = None, stream=None):

@@ -141,9 +141,10 @@ int mss_map_reads_fast(const mss_genome_t* g, const uint32_t* d_reads, const uin
                           workspace_bytes, stream, d_out, 2, nullptr, 0);
 }
 
-int mss_map_reads_bounds(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
-                         const int32_t* d_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands,
-                         int32_t every_other, void* stream, uint16_t* d_bounds, int32_t* h_delta)
+static int bounds_impl(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                       const int32_t* d_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands,
+                       int32_t every_other, void* stream, uint16_t* d_bounds, int32_t* h_delta,
+                       const uint32_t* d_pssm, int32_t pssm_stride)
 {
     if (!g || n_reads < 0 || strands < 1 || strands > 3 || max_len < 1) return MSS_ERR_ARG;
     if (h_delta) *h_delta = 0;
@@ -158,12 +159,29 @@ int mss_map_reads_bounds(const mss_genome_t* g, const uint32_t* d_reads, const u
     p.F = g->frag_len; p.V = g->overlap; p.n_frag = g->n_frag;
     p.reads = d_reads; p.reads_nmask = d_reads_nmask; p.stride_words = read_stride_words; p.lens = d_lens;
     p.n_reads = n_reads; p.max_len = max_len; p.match = sc.match; p.mismatch = sc.mismatch; p.strands = strands; p.zero = 0;
-    p.istep = every_other ? 2 : 1; p.pssm = nullptr; p.pssm_stride = 0; p.ubound = nullptr; p.delta = 0;
+    p.istep = every_other ? 2 : 1; p.pssm = d_pssm; p.pssm_stride = pssm_stride; p.ubound = nullptr; p.delta = 0;
     if (!scan_filter_supported(g, p)) return MSS_ERR_RANGE;
     if (h_delta) *h_delta = scan_filter_delta(p);
     cudaError_t e = launch_scan_filter(g, p, d_bounds, (cudaStream_t)stream, nullptr, nullptr, nullptr, nullptr, nullptr);
     if (e != cudaSuccess) return cuda_fail(e);
     return MSS_OK;
+}
+
+int mss_map_reads_bounds(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                         const int32_t* d_lens, int32_t n_reads, int32_t max_len, mss_scoring_t sc, int32_t strands,
+                         int32_t every_other, void* stream, uint16_t* d_bounds, int32_t* h_delta)
+{
+    return bounds_impl(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, sc, strands, every_other, stream,
+                       d_bounds, h_delta, nullptr, 0);
+}
+
+int mss_map_reads_bounds_pssm(const mss_genome_t* g, const uint32_t* d_reads, const uint32_t* d_reads_nmask, int32_t read_stride_words,
+                              const int32_t* d_lens, int32_t n_reads, int32_t max_len, const uint32_t* d_pssm, int32_t pssm_stride,
+                              mss_scoring_t bound, int32_t strands, void* stream, uint16_t* d_bounds, int32_t* h_delta)
+{
+    if (n_reads > 0 && (!d_pssm || pssm_stride < max_len)) return MSS_ERR_ARG;
+    return bounds_impl(g, d_reads, d_reads_nmask, read_stride_words, d_lens, n_reads, max_len, bound, strands, 0, stream,
+                       d_bounds, h_delta, d_pssm, pssm_stride);
 }
 
 int mss_pssm_build(const uint8_t* d_qual, int32_t qual_stride, const int32_t* d_lens, int32_t n_reads, mss_scoring_t sc,

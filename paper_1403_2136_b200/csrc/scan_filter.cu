@@ -258,10 +258,10 @@ void scan_filter_force_variant(int v, bool tile_kernel) { g_filter_force = v; g_
 
 bool scan_filter_supported(const mss_genome* g, const ScanParams& p)
 {
-    if (p.pssm) return false;                                   // position-specific scores: one-pass scan only
     if (g->frag_len < 256 || g->n_frag < 8) return false;       // nothing to prune
     if ((int64_t)p.max_len * p.match > 32767 || 2 * (int64_t)p.mismatch < -32768 || 2 * (int64_t)p.match > 32767) return false;
     if (!g_filter_tile_kernel && scan_filter_lq_supported(g, p)) return true;
+    if (p.pssm) return false;                                   // position-specific scores: only the lane-per-query kernel bounds them
     return pick_filter_variant(g, p) >= 0;
 }
 

@@ -27,6 +27,14 @@
 //            any scoring whose sums have <= 3 significant bits are exact), four per word = two adjacent columns x two
 //            window starts: one LDS.32 feeds two chains, a PRMT per chain widens a byte pair to fp16x2, then as LQ_F16.
 //            Half the shared-memory wavefronts per cell.
+//   LQ_PSSM  base-quality scoring: every query position has its own (pmatch, pmismatch), so a double step has
+//            four possible operands T[p], p = match pattern of its two positions.  The planes are query-independent as
+//            before but hold, per column and window start, the PRMT SELECTOR of the pattern (byte (2p+1)<<4 | 2p); a
+//            thread loads its own query's T and plane offset of the double step (one LDS.128 from a per-query table,
+//            shared by its 8 chains: the offsets need no registers, so one instance serves every read length) and one
+//            PRMT(T.lo, T.hi, selector) per chain yields the packed int16 operand pair; then VIADDMNMX.S16x2.RELU /
+//            VIMNMX3.S16x2 as LQ_S16 (scores reach scale * match * m: no fp16).  Bound: delta = min(PM, -PMM) - PMM
+//            with PM / PMM the table's largest pmatch / most negative pmismatch.
 #include <cuda_fp16.h>
 #include "mss_common.cuh"
 
@@ -41,7 +49,7 @@ constexpr int LQ_NPL = 21;
 constexpr int LQ_NPL_N = 31;
 constexpr int LQ_ZERO_PLANE = 20;
 constexpr int LQ_MAX_QSETS = 4;
-enum { LQ_S16 = 0, LQ_F16 = 1, LQ_F8 = 2 };
+enum { LQ_S16 = 0, LQ_F16 = 1, LQ_F8 = 2, LQ_PSSM = 3 };
 
 struct LqTile {
     int32_t HALF, ROWW, NG;         // tile = 2*HALF window starts; plane stride (words); column groups per warp and tile
@@ -53,6 +61,7 @@ struct LqGeom {
     int32_t qsets;                  // query sets (of 32 lanes) per block: 1, 2 or 4; a set is scanned by NW / qsets warps
     LqTile a;                       // blocks without an N in their reads: 21 planes
     LqTile b;                       // blocks with one: 31 planes, smaller tile (HALF = 0: none fits, such reads stay unbounded)
+    int32_t tstride;                // PSSM: entries of a thread's double-step table (odd, >= the double steps of the longest read + 1)
 };
 
 __device__ __forceinline__ void lq_cp_async4(void* smem_dst, const void* gmem_src)
@@ -61,10 +70,18 @@ __device__ __forceinline__ void lq_cp_async4(void* smem_dst, const void* gmem_sr
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(d), "l"(gmem_src) : "memory");
 }
 
+// PRMT with a register selector whose nibbles are all < 8 (__byte_perm would mask it with 0x7777 first: one LOP3 per use)
+__device__ __forceinline__ uint32_t lq_prmt(uint32_t a, uint32_t b, uint32_t sel)
+{
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
+    return d;
+}
+
 template <int MODE>
 __device__ __forceinline__ uint32_t lq_enc(int32_t v)            // one lane's operand: int16, or fp16 bits of the integer
 {
-    if (MODE == LQ_S16) return (uint32_t)v & 0xFFFFu;
+    if (MODE == LQ_S16 || MODE == LQ_PSSM) return (uint32_t)v & 0xFFFFu;
     return (uint32_t)__half_as_ushort(__int2half_rn(v));
 }
 
@@ -76,11 +93,15 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
 {
     constexpr int K = LQ_K, NW = LQ_NW, T = 32 * NW;
     constexpr int NREG = PACKED ? NJ / 2 : NJ;
+    constexpr bool BYTEP = (MODE == LQ_F8 || MODE == LQ_PSSM);   // planes hold one byte per (column, window start): two columns per word
+    // PSSM: a query's table of (operands, plane offset) per double step: ug.tstride 16-byte entries (odd: conflict-free LDS.128)
+    const int32_t TABW = (MODE == LQ_PSSM) ? 4 * ug.tstride : 0;
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t* wres = smem;                                      // NW * 32: per (warp, lane) tile maximum
     int32_t* qnj = (int32_t*)(wres + NW * 32);                  // 32 * qsets: double steps of a query; 0 = not scanned
     int32_t* qm = qnj + 32 * LQ_MAX_QSETS;                      // 32 * qsets: read length
-    uint32_t* planes = (uint32_t*)(qm + 32 * LQ_MAX_QSETS);     // NPL * ROWW (the tile geometry is chosen below)
+    uint32_t* tab = (uint32_t*)(qm + 32 * LQ_MAX_QSETS);        // PSSM: 32 * qsets * TABW words, one table per query
+    uint32_t* planes = tab + 32 * ug.qsets * TABW;              // NPL * ROWW (the tile geometry is chosen below)
     uint8_t* sq = reinterpret_cast<uint8_t*>(planes);           // prologue only: strand-oriented base codes, row = query
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -131,17 +152,20 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
     const int32_t CW = HALF / wps;                              // columns of a tile scanned by one warp
     uint32_t* rawp = planes + NPL * ROWW;                       // 2 * NRAW: packed genome words of this tile / the next (cp.async)
     uint32_t* rawn = rawp + 2 * tg.NRAW;                        // 2 * (NRAW / 2 + 1): N-mask words
-    const int32_t words_before = NW * 32 + 2 * 32 * LQ_MAX_QSETS + NPL * ROWW + 2 * tg.NRAW + 2 * (tg.NRAW / 2 + 1);
+    const int32_t words_before = NW * 32 + 2 * 32 * LQ_MAX_QSETS + 32 * ug.qsets * TABW + NPL * ROWW + 2 * tg.NRAW + 2 * (tg.NRAW / 2 + 1);
     uint8_t* codes = reinterpret_cast<uint8_t*>(smem + ((words_before + 3) & ~3));   // 16 * NRAW one-hot base codes (16-byte aligned)
 
     // ---- step 2: this lane's query -> plane offsets in registers -----------------------------------------------------
-    // a column is a word (LQ_S16, LQ_F16) or half a word (LQ_F8: columns 2c, 2c+1 share word c; every offset below is even)
+    // a column is a word (LQ_S16, LQ_F16) or half a word (byte planes: columns 2c, 2c+1 share word c; every offset below is even)
     const int32_t myq = set * 32 + lane;
     const int32_t mynj = qnj[myq], mym = qm[myq];
-    uint32_t off[NREG];
-#pragma unroll
-    for (int j = 0; j < NJ; j++) {
-        uint32_t plane = LQ_ZERO_PLANE, col = 0u;                   // padding step: adds 0
+    const int32_t mystrand = (ns == 2) ? (myq & 1) : (p.strands == 2 ? 1 : 0);
+    const uint32_t* myprow = (MODE == LQ_PSSM && myq < nq) ? p.pssm + (int64_t)(r0 + myq / ns) * p.pssm_stride : nullptr;
+    uint4* mytab_w = reinterpret_cast<uint4*>(tab) + (size_t)myq * ug.tstride;
+    (void)mystrand; (void)myprow; (void)mytab_w;
+    // word offset (plane, column) of the operand of double step j for chain 0 of group 0; padding steps: the zero plane
+    auto step_word = [&](int32_t j) -> uint32_t {
+        uint32_t plane = LQ_ZERO_PLANE, col = 0u;
         if (j < mynj) {
             const int32_t i1 = 2 * j * istep, i2 = i1 + istep;
             const uint32_t b1 = sq[myq * sq_stride + i1];                       // 0..3, 4 = N
@@ -150,12 +174,33 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
             else plane = b2 < 4u ? 25u + b2 : (b2 == 5u ? 30u : 29u);
             col = (uint32_t)i1;
         }
-        const uint32_t cw = col + (uint32_t)(ws * CW);              // column of chain 0, group 0
-        const uint32_t w = plane * (uint32_t)ROWW + (MODE == LQ_F8 ? cw >> 1 : cw);
-        if (PACKED) {
-            if (j & 1) off[j >> 1] |= w << 16; else off[j >> 1] = w;
-        } else {
-            off[j] = w * 4u;
+        const uint32_t cw = col + (MODE == LQ_PSSM ? 0u : (uint32_t)(ws * CW));     // column of chain 0, group 0 (PSSM: of warp 0)
+        return plane * (uint32_t)ROWW + (BYTEP ? cw >> 1 : cw);
+    };
+    uint32_t off[NREG];
+    if (MODE != LQ_PSSM) {
+#pragma unroll
+        for (int j = 0; j < NJ; j++) {
+            const uint32_t w = step_word(j);
+            if (PACKED) {
+                if (j & 1) off[j >> 1] |= w << 16; else off[j >> 1] = w;
+            } else {
+                off[j] = w * 4u;
+            }
+        }
+    } else {
+        // PSSM: the offsets live next to the query's operands in its shared-memory table, one 16-byte entry per double step,
+        // written by the first warp of the query's set and shared by the others (whose column share goes into the group base)
+        for (int32_t j = 0; j < (ws == 0 ? ug.tstride : 0); j++) {
+            uint32_t t01 = 0u, t23 = 0u;
+            if (j < mynj) {
+                const int32_t i1 = 2 * j, i2 = i1 + 1;
+                const uint32_t w1 = pssm_at(myprow, mym, i1, mystrand), w2 = (i2 < mym) ? pssm_at(myprow, mym, i2, mystrand) : 0u;
+                const int32_t pm1 = (int16_t)(w1 & 0xFFFFu), px1 = (int16_t)(w1 >> 16), pm2 = (int16_t)(w2 & 0xFFFFu), px2 = (int16_t)(w2 >> 16);
+                t01 = ((uint32_t)(px1 + px2) & 0xFFFFu) | ((uint32_t)(pm1 + px2) << 16);      // patterns 0 (neither), 1 (first matches)
+                t23 = ((uint32_t)(px1 + pm2) & 0xFFFFu) | ((uint32_t)(pm1 + pm2) << 16);      // 2 (second), 3 (both)
+            }
+            mytab_w[j] = make_uint4(t01, t23, step_word(j) * 4u, 0u);
         }
     }
     // double steps this warp runs: the longest query of its set, rounded up to the pair the loop body handles
@@ -168,6 +213,8 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
     const uint32_t e2_0 = lq_enc<MODE>(2 * X), e2_1 = lq_enc<MODE>(M + X), e2_2 = lq_enc<MODE>(2 * M);
     const uint32_t e1_0 = lq_enc<MODE>(X), e1_1 = lq_enc<MODE>(M);
     const char* planes_b = reinterpret_cast<const char*>(planes);
+    const uint4* mytab = reinterpret_cast<const uint4*>(tab) + (size_t)myq * ug.tstride;
+    (void)mytab;
     uint32_t cur = 0u;                                              // fold threads (tid < 32 * qsets): running fragment maximum
     int32_t prev_f = -1; bool prev_last = false;
 
@@ -181,7 +228,7 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
             if (tid < nq) {
                 const int32_t r = r0 + tid / ns, s = tid % ns;
                 uint32_t u = c;                                     // fp16 modes: bit pattern of a non-negative integer value
-                if (MODE != LQ_S16) u = (uint32_t)__half2int_rn(__ushort_as_half((unsigned short)c));
+                if (MODE == LQ_F16 || MODE == LQ_F8) u = (uint32_t)__half2int_rn(__ushort_as_half((unsigned short)c));
                 ubound[((int64_t)r * ns + s) * p.n_frag + prev_f] = (qnj[tid] == 0) ? (uint16_t)0xFFFFu : (uint16_t)u;
             }
             c = 0u;
@@ -240,7 +287,7 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
             __syncthreads();
             // ---- a2: codes -> dibase planes ----------------------------------------------------------------------
             const int32_t sh = (int32_t)(g0 & 15);                  // codes[sh + x] = genome position g0 + x
-            if (MODE != LQ_F8) {
+            if (!BYTEP) {
                 for (int32_t x = tid; x < tg.COLS; x += T) {
                     const uint32_t lo1 = codes[sh + x], lo2 = codes[sh + x + istep];
                     const uint32_t hi1 = codes[sh + x + HALF], hi2 = codes[sh + x + HALF + istep];
@@ -267,8 +314,10 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                 // nibbles of a 16-bit value; (OH >> c) & 0x1111 is then the lanes' match flag against base c, the sum of two
                 // such values their match count (0..2 per nibble), and one PRMT with that value as the selector maps every
                 // count to its operand byte: 3 instructions per plane word
-                const uint32_t tab2 = (e2_0 >> 8) | (e2_1 & 0xFF00u) | ((e2_2 & 0xFF00u) << 8);
-                const uint32_t tab1 = (e1_0 >> 8) | (e1_1 & 0xFF00u);
+                // PSSM: the byte is the PRMT selector of the match pattern p = first + 2 * second, (2p + 1) << 4 | 2p
+                const uint32_t tab2 = MODE == LQ_PSSM ? 0x76543210u : (e2_0 >> 8) | (e2_1 & 0xFF00u) | ((e2_2 & 0xFF00u) << 8);
+                const uint32_t tab1 = MODE == LQ_PSSM ? 0x76543210u : (e1_0 >> 8) | (e1_1 & 0xFF00u);
+                const uint32_t second = MODE == LQ_PSSM ? 2u : 1u;  // weight of the second position in the table index
                 for (int32_t xw = tid; xw < tg.COLS / 2; xw += T) {
                     const uint8_t* c0 = codes + sh + 2 * xw;
                     const uint32_t oh1 = c0[0] | (c0[HALF] << 4) | (c0[1] << 8) | (c0[HALF + 1] << 12);
@@ -280,15 +329,18 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                     for (uint32_t c1 = 0; c1 < 4; c1++) {
 #pragma unroll
                         for (uint32_t c2 = 0; c2 < 4; c2++)
-                            planes[(c1 * 4 + c2) * ROWW + xw] = __byte_perm(tab2, 0u, A[c1] + Bm[c2]);
-                        planes[(16 + c1) * ROWW + xw] = __byte_perm(tab1, 0u, A[c1]);
+                            planes[(c1 * 4 + c2) * ROWW + xw] = lq_prmt(tab2, 0u, A[c1] + second * Bm[c2]);
+                        planes[(16 + c1) * ROWW + xw] = lq_prmt(tab1, 0u, A[c1]);
                         if (with_n) {                               // (c1, N): the second position never matches; (N, c): the first
-                            planes[(21 + c1) * ROWW + xw] = __byte_perm(tab2, 0u, A[c1]);
-                            planes[(25 + c1) * ROWW + xw] = __byte_perm(tab2, 0u, Bm[c1]);
+                            planes[(21 + c1) * ROWW + xw] = lq_prmt(tab2, 0u, A[c1]);
+                            planes[(25 + c1) * ROWW + xw] = lq_prmt(tab2, 0u, second * Bm[c1]);
                         }
                     }
-                    planes[LQ_ZERO_PLANE * ROWW + xw] = 0u;
-                    if (with_n) { planes[29 * ROWW + xw] = (e2_0 >> 8) * 0x01010101u; planes[30 * ROWW + xw] = (e1_0 >> 8) * 0x01010101u; }
+                    planes[LQ_ZERO_PLANE * ROWW + xw] = MODE == LQ_PSSM ? 0x10101010u : 0u;      // PSSM: pattern 0 of an all-zero table
+                    if (with_n) {
+                        planes[29 * ROWW + xw] = MODE == LQ_PSSM ? 0x10101010u : (e2_0 >> 8) * 0x01010101u;
+                        planes[30 * ROWW + xw] = MODE == LQ_PSSM ? 0x10101010u : (e1_0 >> 8) * 0x01010101u;
+                    }
                 }
             }
             __syncthreads();
@@ -296,23 +348,21 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
             // ---- a3: this lane's query against the warp's columns of the tile --------------------------------------
             uint32_t tmax = 0u;
             for (int32_t g = 0; g < tg.NG; g++) {
-                const char* pg = planes_b + g * (MODE == LQ_F8 ? K * 2 : K * 4);    // warp-uniform group base
+                const char* pg = planes_b + g * (BYTEP ? K * 2 : K * 4) + (MODE == LQ_PSSM ? ws * CW * 2 : 0);   // warp-uniform group base
                 uint32_t H[K], B[K];
 #pragma unroll
                 for (int k = 0; k < K; k++) { H[k] = 0u; B[k] = 0u; }
-#pragma unroll
-                for (int j = 0; j < NJ; j += 2) {
-                    if ((j & 7) == 0 && j >= njb) break;            // padding steps add 0: the check only saves time, so it is coarse
-                    uint32_t o0, o1;
-                    if (PACKED) {                                   // volatile: unpacked per use, or the compiler hoists all NJ results out of the group loop and spills them
-                        uint32_t lo, hi;
-                        asm volatile("and.b32 %0, %1, 0xFFFF;" : "=r"(lo) : "r"(off[j >> 1]));
-                        asm volatile("shr.u32 %0, %1, 16;" : "=r"(hi) : "r"(off[j >> 1]));
-                        o0 = lo << 2; o1 = hi << 2;
-                    }
-                    else { o0 = off[j]; o1 = off[j + 1]; }
+                // two double steps of the K chains: operands at byte offsets o0, o1 of the group's columns (PSSM: tq = the
+                // query's four operands of either double step)
+                auto pair = [&](uint32_t o0, uint32_t o1, const uint4& tq) {
                     uint32_t Ha[K], v[K];
-                    if (MODE == LQ_F8) {
+                    if (MODE == LQ_PSSM) {
+#pragma unroll
+                        for (int k = 0; k < K; k += 2) {
+                            const uint32_t w = *reinterpret_cast<const uint32_t*>(pg + o0 + k * 2);
+                            v[k] = lq_prmt(tq.x, tq.y, w); v[k + 1] = lq_prmt(tq.x, tq.y, w >> 16);
+                        }
+                    } else if (MODE == LQ_F8) {
 #pragma unroll
                         for (int k = 0; k < K; k += 2) {
                             const uint32_t w = *reinterpret_cast<const uint32_t*>(pg + o0 + k * 2);
@@ -324,10 +374,16 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                     }
 #pragma unroll
                     for (int k = 0; k < K; k++) {
-                        if (MODE == LQ_S16) Ha[k] = __viaddmax_s16x2(H[k], v[k], zero);
+                        if (MODE == LQ_S16 || MODE == LQ_PSSM) Ha[k] = __viaddmax_s16x2(H[k], v[k], zero);
                         else asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(Ha[k]) : "r"(H[k]), "r"(0x3C003C00u), "r"(v[k]));
                     }
-                    if (MODE == LQ_F8) {
+                    if (MODE == LQ_PSSM) {
+#pragma unroll
+                        for (int k = 0; k < K; k += 2) {
+                            const uint32_t w = *reinterpret_cast<const uint32_t*>(pg + o1 + k * 2);
+                            v[k] = lq_prmt(tq.z, tq.w, w); v[k + 1] = lq_prmt(tq.z, tq.w, w >> 16);
+                        }
+                    } else if (MODE == LQ_F8) {
 #pragma unroll
                         for (int k = 0; k < K; k += 2) {
                             const uint32_t w = *reinterpret_cast<const uint32_t*>(pg + o1 + k * 2);
@@ -339,11 +395,33 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                     }
 #pragma unroll
                     for (int k = 0; k < K; k++) {
-                        if (MODE == LQ_S16) H[k] = __viaddmax_s16x2(Ha[k], v[k], zero);
+                        if (MODE == LQ_S16 || MODE == LQ_PSSM) H[k] = __viaddmax_s16x2(Ha[k], v[k], zero);
                         else asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(H[k]) : "r"(Ha[k]), "r"(0x3C003C00u), "r"(v[k]));
                     }
 #pragma unroll
                     for (int k = 0; k < K; k++) B[k] = __vimax3_s16x2(B[k], Ha[k], H[k]);
+                };
+                if (MODE == LQ_PSSM) {
+                    // the query's table entry of a double step = (operands 0/1, operands 2/3, plane offset, -): one LDS.128
+#pragma unroll 2
+                    for (int32_t j = 0; j < njb; j += 2) {
+                        const uint4 ta = mytab[j], tb = mytab[j + 1];
+                        pair(ta.z, tb.z, make_uint4(ta.x, ta.y, tb.x, tb.y));
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < NJ; j += 2) {
+                        if ((j & 7) == 0 && j >= njb) break;        // padding steps add 0: the check only saves time, so it is coarse
+                        uint32_t o0, o1;
+                        if (PACKED) {                               // volatile: unpacked per use, or the compiler hoists all NJ results out of the group loop and spills them
+                            uint32_t lo, hi;
+                            asm volatile("and.b32 %0, %1, 0xFFFF;" : "=r"(lo) : "r"(off[j >> 1]));
+                            asm volatile("shr.u32 %0, %1, 16;" : "=r"(hi) : "r"(off[j >> 1]));
+                            o0 = lo << 2; o1 = hi << 2;
+                        }
+                        else { o0 = off[j]; o1 = off[j + 1]; }
+                        pair(o0, o1, make_uint4(0u, 0u, 0u, 0u));
+                    }
                 }
                 if (nvalid < D) {                                   // ragged last tile of a fragment: drop foreign window starts
                     const int32_t x0 = ws * CW + g * K;
@@ -375,19 +453,26 @@ bool lq_e5m2_exact(int32_t v)
 }
 
 struct LqSmem { int32_t ROWW, COLS, NRAW; size_t bytes; };
-LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode, int npl)
+// PSSM: table entries per thread: the double steps of the longest read, rounded up to the pair the loop handles, made odd
+int32_t lq_tstride(int32_t max_len, int32_t istep)
+{
+    int32_t steps = (max_len + istep - 1) / istep;
+    return ((((steps + 1) / 2) + 1) & ~1) | 1;
+}
+LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode, int npl, int32_t qsets)
 {
     // columns read: chain column < HALF, plus the column of the last double step (< max_len rounded up to even steps)
     LqSmem s;
     int32_t halo = ((max_len + 2 * istep + 3) & ~3);
     s.COLS = half + halo;
-    int32_t roww = mode == LQ_F8 ? s.COLS / 2 : s.COLS;
+    int32_t roww = (mode == LQ_F8 || mode == LQ_PSSM) ? s.COLS / 2 : s.COLS;
     roww += (33 - (roww & 31)) & 31;                            // 1 (mod 32): plane p, word c -> bank (p + c) mod 32
     s.ROWW = roww;
     // genome positions a tile reads: [g0, g0 + HALF + COLS + istep), from the 16-aligned position below g0
     s.NRAW = ((half + s.COLS + istep + 15 + 15) / 16 + 1) & ~1;
     // planes, wres, qnj + qm, raw words (2 buffers), raw mask words (2 buffers), pad to 16 bytes, codes
     size_t words = (size_t)npl * roww + LQ_NW * 32 + 2 * 32 * LQ_MAX_QSETS + 2 * s.NRAW + 2 * (s.NRAW / 2 + 1);
+    if (mode == LQ_PSSM) words += (size_t)32 * qsets * 4 * lq_tstride(max_len, istep);     // per-query (operands, offset) tables
     words = (words + 3) & ~(size_t)3;
     s.bytes = words * 4 + (size_t)16 * s.NRAW;
     return s;
@@ -399,6 +484,7 @@ thread_local int t_lq_mode = -1;       // tuning hook: force the arithmetic (-1 
 
 int lq_mode(const ScanParams& p)
 {
+    if (p.pssm) return LQ_PSSM;
     const int32_t M = p.match, X = p.mismatch;
     const bool f16_ok = (int64_t)p.max_len * M <= 2048 && 2 * M <= 2048 && -2 * X <= 2048;
     const bool f8_ok = f16_ok && lq_e5m2_exact(2 * M) && lq_e5m2_exact(M + X) && lq_e5m2_exact(2 * X) && lq_e5m2_exact(M) &&
@@ -419,7 +505,7 @@ bool lq_pick_tile(const mss_genome* g, const ScanParams& p, int32_t qsets, int m
     for (int32_t half = unit; half <= 4096; half += unit) {
         if (forced_half > 0 && half != forced_half) continue;
         if (half < 128) continue;
-        LqSmem s = lq_smem(half, p.max_len, p.istep, mode, npl);
+        LqSmem s = lq_smem(half, p.max_len, p.istep, mode, npl, qsets);
         if (s.bytes * 2 + 4096 > (size_t)g->max_smem_optin) break;
         if ((size_t)npl * s.ROWW * 4 < prologue) continue;         // the prologue borrows the plane area
         if ((int64_t)npl * s.ROWW + 4096 > 65535) break;             // packed 16-bit word offsets
@@ -429,7 +515,7 @@ bool lq_pick_tile(const mss_genome* g, const ScanParams& p, int32_t qsets, int m
         if (waste < best_waste - 1e-9) { best_waste = waste; best = half; }
     }
     if (!best) return false;
-    LqSmem s = lq_smem(best, p.max_len, p.istep, mode, npl);
+    LqSmem s = lq_smem(best, p.max_len, p.istep, mode, npl, qsets);
     if (out) { out->HALF = best; out->ROWW = s.ROWW; out->COLS = s.COLS; out->NRAW = s.NRAW; out->NG = best / unit; }
     if (bytes) *bytes = s.bytes;
     return true;
@@ -442,7 +528,7 @@ bool lq_pick(const mss_genome* g, const ScanParams& p, int32_t qsets, int mode, 
     size_t ba = 0, bb = 0;
     if (!lq_pick_tile(g, p, qsets, mode, LQ_NPL, t_lq_half, &a, &ba)) return false;
     if (!lq_pick_tile(g, p, qsets, mode, LQ_NPL_N, 0, &b, &bb)) { b = LqTile{0, 0, 0, 0, 0}; bb = 0; }
-    if (out) { out->a = a; out->b = b; out->qsets = qsets; }
+    if (out) { out->a = a; out->b = b; out->qsets = qsets; out->tstride = lq_tstride(p.max_len, p.istep); }
     if (bytes) *bytes = ba > bb ? ba : bb;
     return true;
 }
@@ -451,9 +537,25 @@ bool lq_pick(const mss_genome* g, const ScanParams& p, int32_t qsets, int mode, 
 // cells/clk/SM with 1 / 2 / 4 sets), fewer keep the grid fine for small batches
 int32_t lq_qsets(const ScanParams& p)
 {
+    if (p.pssm) return 1;                                       // the per-query tables take the room more query sets would need
     if (t_lq_qsets) return t_lq_qsets;
     const int64_t queries = (int64_t)p.n_reads * (p.strands == 3 ? 2 : 1);
     return queries >= 65536 ? 4 : (queries >= 16384 ? 2 : 1);
+}
+
+// the kernel instance (most double steps held) that serves queries of up to nj double steps
+int32_t lq_nj_instance(int32_t nj, int mode)
+{
+    if (mode == LQ_F8) {
+        if (nj <= 18) return 18;
+        if (nj <= 26) return 26;
+        if (nj > 32 && nj <= 38) return 38;
+    }
+    if (mode == LQ_F8 && nj > 38 && nj <= 50) return 50;
+    if (nj <= 32) return 32;
+    if (nj <= 64) return 64;
+    if (nj <= 80) return 80;
+    return 128;
 }
 
 int32_t lq_double_steps(const ScanParams& p)
@@ -491,6 +593,7 @@ void scan_filter_lq_tune(int qsets, int half, int mode)
 
 bool scan_filter_lq_supported(const mss_genome* g, const ScanParams& p)
 {
+    if (p.pssm && p.istep != 1) return false;
     if (lq_double_steps(p) > 128) return false;                 // longer queries: the tile kernel of scan_filter.cu
     return lq_pick(g, p, lq_qsets(p), lq_mode(p), nullptr, nullptr);
 }
@@ -517,17 +620,18 @@ cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint
     if (smem_out) *smem_out = (int32_t)smem;
     if (tile_out) *tile_out = 2 * ug.a.HALF;
     if (rpb_out) *rpb_out = ug.reads_per_group;
-    const int32_t nj = lq_double_steps(p);
     // padding steps cost time (the early-exit check is coarse): the common read lengths get a tight instance of the
     // fast arithmetic (36, 51, 76, 100 bp)
-    if (mode == LQ_F8) {
-        if (nj <= 18) return lq_launch3<18, false, LQ_F8>(p, ug, ubound, st, smem);
-        if (nj <= 26) return lq_launch3<26, false, LQ_F8>(p, ug, ubound, st, smem);
-        if (nj > 32 && nj <= 38) return lq_launch3<38, false, LQ_F8>(p, ug, ubound, st, smem);
-        if (nj > 38 && nj <= 50) return lq_launch3<50, false, LQ_F8>(p, ug, ubound, st, smem);
+    if (mode == LQ_PSSM) return lq_launch3<2, false, LQ_PSSM>(p, ug, ubound, st, smem);   // table-driven: one instance for every length
+    switch (lq_nj_instance(lq_double_steps(p), mode)) {
+        case 18: return lq_launch3<18, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 26: return lq_launch3<26, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 38: return lq_launch3<38, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 50: return lq_launch3<50, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 32: return lq_launch<32, false>(mode, p, ug, ubound, st, smem);
+        case 64: return lq_launch<64, false>(mode, p, ug, ubound, st, smem);
+        case 80: return lq_launch<80, false>(mode, p, ug, ubound, st, smem);
+        default: break;
     }
-    if (nj <= 32) return lq_launch<32, false>(mode, p, ug, ubound, st, smem);
-    if (nj <= 64) return lq_launch<64, false>(mode, p, ug, ubound, st, smem);
-    if (nj <= 80) return lq_launch<80, false>(mode, p, ug, ubound, st, smem);
     return lq_launch<128, true>(mode, p, ug, ubound, st, smem);
 }

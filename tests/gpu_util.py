@@ -74,7 +74,7 @@ def pssm_tables(quals, lens, match=5, mismatch=-4, scale=16):
     return d, pm, pmm
 
 
-def map_reads_pssm(g, reads, lens, d_pssm, strands=3, match=5, mismatch=-4, scale=16, variant=0):
+def map_reads_pssm(g, reads, lens, d_pssm, strands=3, match=5, mismatch=-4, scale=16, variant=0, bound=None):
     import torch
     import paper_1403_2136_b200 as mss
     reads = np.asarray(reads, dtype=np.uint8)
@@ -83,7 +83,7 @@ def map_reads_pssm(g, reads, lens, d_pssm, strands=3, match=5, mismatch=-4, scal
     mss.mss_set_scan_variant(variant)
     try:
         out = mss.mss_map_reads_pssm(g, to_dev(rp), to_dev(rn), to_dev(lens), int(reads.shape[1]), d_pssm,
-                                     mss.pssm_bound(mss.Scoring(match, mismatch, -26), scale), strands)
+                                     bound or mss.pssm_bound(mss.Scoring(match, mismatch, -26), scale), strands)
         torch.cuda.synchronize()
     finally:
         mss.mss_set_scan_variant(0)

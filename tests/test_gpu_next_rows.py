@@ -144,7 +144,8 @@ def test_pssm_uniform_table_equals_plain_scan(tiny):
     d_pssm = to_dev(np.full(reads.shape, w, dtype=np.uint32))
     G = load_genome(g, cfg.frag_len, -1)
     a = map_reads(G, reads, lens, strands=3)
-    b = map_reads_pssm(G, reads, lens, d_pssm, strands=3, scale=1)
+    import paper_1403_2136_b200 as mss
+    b = map_reads_pssm(G, reads, lens, d_pssm, strands=3, bound=mss.Scoring(5, -4, -26))     # a hand-made table states its own range
     torch.cuda.synchronize()
     _cmp(b, a, "uniform table")
 
@@ -198,3 +199,73 @@ def test_next_row_argument_errors(tiny):
         mss.mss_map_reads_pssm(G, to_dev(rp), to_dev(rn), to_dev(lens[:4]), 100, d_p[:, :50].contiguous(),
                                mss.pssm_bound(mss.Scoring(), 16), 3)
     assert e.value.status == -1
+
+
+def _pssm_fragment_scores(oracle_mod, g, F, V, q, m, pm, pmm):
+    """Exact per-fragment PSSM scores of one strand-oriented query (q, pm, pmm already oriented): the pinned PSSM oracle on
+    a genome cut to each fragment's readable window (one fragment, forward strand)."""
+    nfrag = -(-g.size // F)
+    out = np.zeros(nfrag, dtype=np.int64)
+    veff = m - 1 if (V < 0 or V > m - 1) else V
+    for f in range(nfrag):
+        sub = g[f * F: min(g.size, f * F + F + veff)]
+        padn = np.full(F + veff, gen.N, dtype=np.uint8); padn[:sub.size] = sub
+        r = oracle_mod.map_reads_pssm(padn, F, veff, q[None, :m], [m], pm[None, :m], pmm[None, :m], strands=1)
+        out[f] = r[0, 0, 2] if r[0, 0, 0] == 0 else (r[0, 1, 2] if r[0, 1, 0] == 0 else 0)
+    return out
+
+
+@pytest.mark.parametrize("F,V,m,scale", [(1000, -1, 100, 16), (1000, 0, 75, 16), (700, 30, 51, 8), (2048, -1, 150, 16)])
+def test_pssm_pass1_bounds_hold(oracle_mod, F, V, m, scale):
+    """Pass 1 under base-quality scoring (scan_filter_lq_kernel, PSSM form): u <= exact <= u + delta for every read, strand
+    and fragment against the oracle's PSSM scores, reads with N, ragged lengths and Q2 tails included."""
+    import torch
+    import paper_1403_2136_b200 as mss
+    from gpu_util import load_genome, pssm_tables, to_dev
+    g = gen.make_genome(24_000, 41)[0]
+    g[3000:3200] = gen.N
+    r = gen.make_reads(g, 20, m, 4100 + m, sub_rate=0.15)
+    reads, lens = r["reads"].copy(), r["lens"].copy()
+    lens[4] = m - 9; reads[4, lens[4]:] = gen.N
+    lens[6] = 1; reads[6, 1:] = gen.N
+    reads[2, m // 3] = gen.N
+    reads[11, m // 2: m // 2 + 3] = gen.N
+    quals = gen.make_quals(20, m, 4200 + m)
+    d_pssm, _, _ = pssm_tables(quals, lens, scale=scale)
+    pm, pmm = oracle_mod.pssm_from_phred(quals, 5, -4, scale)            # the oracle's own table feeds the oracle
+    G = load_genome(g, F, V)
+    rp, rn = gen.pack_reads(reads, lens)
+    bound = mss.pssm_bound(mss.Scoring(), scale)
+    u, delta = mss.mss_map_reads_bounds_pssm(G, to_dev(rp), to_dev(rn), to_dev(lens), m, d_pssm, bound, 3)
+    torch.cuda.synchronize()
+    u = u.cpu().numpy().view(np.uint16).astype(np.int64)
+    assert delta == min(bound.match, -bound.mismatch) - bound.mismatch
+    assert pm.max() <= bound.match and pmm.min() >= bound.mismatch       # the stated range holds for the oracle's table
+    for i in range(reads.shape[0]):
+        mi = int(lens[i])
+        for s in (0, 1):
+            q = gen.revcomp(reads[i, :mi]) if s else reads[i, :mi]
+            a, b = (pm[i, :mi][::-1], pmm[i, :mi][::-1]) if s else (pm[i, :mi], pmm[i, :mi])
+            ex = _pssm_fragment_scores(oracle_mod, g, F, V, q, mi, np.ascontiguousarray(a), np.ascontiguousarray(b))
+            assert (u[i, s] != 0xFFFF).all()
+            assert (u[i, s] <= ex).all() and (ex <= u[i, s] + delta).all(), (i, s, int(np.argmax(np.abs(ex - u[i, s]))))
+
+
+def test_pssm_takes_the_two_pass_scan(oracle_mod, tiny):
+    """The automatic PSSM scan is the two-pass scan (pass 1 in its PSSM form), with records identical to the oracle's; a
+    read with an N and the tile kernel request (variant 13: no PSSM pass 1 there) fall back without changing the records."""
+    import paper_1403_2136_b200 as mss
+    from gpu_util import load_genome, map_reads_pssm, pssm_tables
+    cfg, g, reads, lens, quals = tiny
+    reads = reads.copy()
+    reads[3, 50] = gen.N
+    d_pssm, _, _ = pssm_tables(quals, lens)
+    wpm, wpmm = oracle_mod.pssm_from_phred(quals, 5, -4, 16)
+    want = oracle_mod.map_reads_pssm_parallel(g, cfg.frag_len, -1, reads, lens, wpm, wpmm, strands=3)
+    G = load_genome(g, cfg.frag_len, -1)
+    got = map_reads_pssm(G, reads, lens, d_pssm, strands=3)
+    info = mss.mss_get_last_launch()
+    assert info["variant"] == 7 and info["pass1_kernel"] == 5
+    _cmp(got, want, "pssm two-pass")
+    _cmp(map_reads_pssm(G, reads, lens, d_pssm, strands=3, variant=13), want, "pssm, tile kernel requested")
+    assert mss.mss_get_last_launch()["pass1_kernel"] == 0
