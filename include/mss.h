@@ -241,7 +241,7 @@ int mss_version(void);                         /* 100*major + minor */
  * Tuning / introspection (does not change results): select the scan kernel variant (0 = automatic: the two-pass scan
  * where the geometry allows it, else the one-pass tile kernel, else the generic kernel; 1 = generic; 2-6 = one-pass tile
  * kernels (K, T) = (8,256), (8,128), (8,64), (4,256), (16,128); 7 = two-pass, same as automatic: pass 1 is the
- * lane-per-query kernel for reads of up to 512 scored positions, else the tile kernel; 8-12 = two-pass with pass 1 = the
+ * lane-per-query kernel for reads of up to 256 scored positions, else the tile kernel; 8-12 = two-pass with pass 1 = the
  * tile kernel and its tile (K, T) = (4,256), (4,128), (4,64), (8,128), (8,256) forced; 13 = two-pass with the tile kernel
  * and its own choice of tile; anything else: MSS_ERR_ARG) and report the
  * launch geometry of the last mss_map_reads call on this thread (two-pass: variant 7, grid / smem_bytes / tile_diagonals of

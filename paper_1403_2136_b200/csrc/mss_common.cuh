@@ -116,7 +116,7 @@ int32_t scan_filter_delta(const ScanParams& p);
 void scan_filter_force_variant(int v, bool tile_kernel);
 cudaError_t launch_scan_filter(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
                                int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out, int32_t* kind_out);
-// pass 1 in the lane-per-query layout (scan_filter_lq.cu): reads of up to 512 scored positions
+// pass 1 in the lane-per-query layout (scan_filter_lq.cu): reads of up to 256 scored positions
 bool scan_filter_lq_supported(const mss_genome* g, const ScanParams& p);
 void scan_filter_lq_tune(int qsets, int half, int mode);
 cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
