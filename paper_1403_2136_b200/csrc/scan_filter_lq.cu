@@ -41,7 +41,13 @@
 namespace {
 
 constexpr int LQ_NW = 8;            // warps per block
-constexpr int LQ_K = 8;             // adjacent columns (chains) per thread and column group
+#ifndef LQ_K_CHAINS
+#define LQ_K_CHAINS 8
+#endif
+#ifndef LQ_BLOCKS_PER_SM
+#define LQ_BLOCKS_PER_SM 2
+#endif
+constexpr int LQ_K = LQ_K_CHAINS;   // adjacent columns (chains) per thread and column group
 // planes of a tile: (c1, c2) -> c1*4 + c2; (c1, pad) -> 16 + c1 (last step of an odd-length query); 20 = all zero (padding
 // steps).  Blocks whose reads hold an N ("N" scores mismatch against everything, reading 6) add ten more:
 // (c1, N) -> 21 + c1, (N, c2) -> 25 + c2, (N, N) -> 29, (N, pad) -> 30, and take a smaller tile to make room for them.
@@ -88,7 +94,7 @@ __device__ __forceinline__ uint32_t lq_enc(int32_t v)            // one lane's o
 // NJ     = most double steps of a query this instantiation holds (even)
 // PACKED = two 16-bit word offsets per register (long reads) instead of one byte offset per register
 template <int NJ, bool PACKED, int MODE>
-__global__ void __launch_bounds__(32 * LQ_NW, 2)
+__global__ void __launch_bounds__(32 * LQ_NW, LQ_BLOCKS_PER_SM)
 scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
 {
     constexpr int K = LQ_K, NW = LQ_NW, T = 32 * NW;
@@ -506,7 +512,7 @@ bool lq_pick_tile(const mss_genome* g, const ScanParams& p, int32_t qsets, int m
         if (forced_half > 0 && half != forced_half) continue;
         if (half < 128) continue;
         LqSmem s = lq_smem(half, p.max_len, p.istep, mode, npl, qsets);
-        if (s.bytes * 2 + 4096 > (size_t)g->max_smem_optin) break;
+        if (s.bytes * LQ_BLOCKS_PER_SM + 2048 * LQ_BLOCKS_PER_SM > (size_t)g->max_smem_optin) break;
         if ((size_t)npl * s.ROWW * 4 < prologue) continue;         // the prologue borrows the plane area
         if ((int64_t)npl * s.ROWW + 4096 > 65535) break;             // packed 16-bit word offsets
         int32_t D = 2 * half;
