@@ -84,6 +84,14 @@ __device__ __forceinline__ uint32_t lq_prmt(uint32_t a, uint32_t b, uint32_t sel
     return d;
 }
 
+// x >> 16 on the FMA pipe (IMAD.HI by 2^16): the PSSM form is bound by the ALU pipe, where SHF would go
+__device__ __forceinline__ uint32_t lq_hi16(uint32_t x)
+{
+    uint32_t d;
+    asm("mul.hi.u32 %0, %1, 65536;" : "=r"(d) : "r"(x));
+    return d;
+}
+
 template <int MODE>
 __device__ __forceinline__ uint32_t lq_enc(int32_t v)            // one lane's operand: int16, or fp16 bits of the integer
 {
@@ -366,7 +374,7 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
 #pragma unroll
                         for (int k = 0; k < K; k += 2) {
                             const uint32_t w = *reinterpret_cast<const uint32_t*>(pg + o0 + k * 2);
-                            v[k] = lq_prmt(tq.x, tq.y, w); v[k + 1] = lq_prmt(tq.x, tq.y, w >> 16);
+                            v[k] = lq_prmt(tq.x, tq.y, w); v[k + 1] = lq_prmt(tq.x, tq.y, lq_hi16(w));
                         }
                     } else if (MODE == LQ_F8) {
 #pragma unroll
@@ -387,7 +395,7 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
 #pragma unroll
                         for (int k = 0; k < K; k += 2) {
                             const uint32_t w = *reinterpret_cast<const uint32_t*>(pg + o1 + k * 2);
-                            v[k] = lq_prmt(tq.z, tq.w, w); v[k + 1] = lq_prmt(tq.z, tq.w, w >> 16);
+                            v[k] = lq_prmt(tq.z, tq.w, w); v[k + 1] = lq_prmt(tq.z, tq.w, lq_hi16(w));
                         }
                     } else if (MODE == LQ_F8) {
 #pragma unroll
