@@ -35,6 +35,8 @@ SMEM_BYTES_PER_CLK_SM = 128         # shared-memory data pipe: one 128-byte wave
 NCU_CAPTURES = {
     "scan_filter_lq_kernel": {"dram_bytes": 2_073_088, "instr_per_cell": 0.828, "smem_bytes_per_cell": 0.5,
                               "source": "profiles/r2_scan_filter_lq_full.md"},
+    "scan_filter_lq_kernel_pssm": {"dram_bytes": 3_751_424, "instr_per_cell": 1.044, "smem_bytes_per_cell": 1.0,
+                                   "source": "profiles/r2_other_kernels.md"},
     "scan_filter_kernel": {"dram_bytes": 2_019_072, "instr_per_cell": 0.871, "smem_bytes_per_cell": 1.0,
                            "source": "profiles/r1_scan_filter_full.md"},
     "scan_dpx_kernel": {"dram_bytes": 2_043_648, "instr_per_cell": 1.54, "smem_bytes_per_cell": 2.0,
@@ -387,10 +389,10 @@ def main():
         kernel = "scan_dpx_kernel"
         kname, kernel_ms, algo = kernel, scan_avg_ms, ALGO_INSTR_PER_CELL
         traffic_model = (genome_bytes + h_reads.numel() * 4) if l2_resident else None
-    cap = NCU_CAPTURES[kernel]
+    cap = NCU_CAPTURES[kernel + ("_pssm" if two_pass and launch_info["pass1_kernel"] == 5 else "")]
     cells_per_clk_sm = cells_step / (kernel_ms * 1e-3) / n_sm / clk
     achieved = cells_step * algo / (kernel_ms * 1e-3)
-    same_launch_as_capture = (args.config == 2 and n_reads == 4096 and args.mode == "plain" and m == 100)
+    same_launch_as_capture = (args.config == 2 and n_reads == 4096 and args.mode in ("plain", "pssm") and m == 100 and args.n_frac == 0)
     roofline = {
         "bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": peak_instr / 1e12, "unit": "T thread-instr/s",
         "frac": achieved / peak_instr,
@@ -412,7 +414,8 @@ def main():
         "issue_frac": cells_per_clk_sm * cap["instr_per_cell"] / ISSUE_LANES_PER_CLK_SM,
         "smem_frac": cells_per_clk_sm * cap["smem_bytes_per_cell"] / SMEM_BYTES_PER_CLK_SM,
         "instr_per_cell_profiled": cap["instr_per_cell"], "smem_bytes_per_cell": cap["smem_bytes_per_cell"],
-        "limiter": ("issue slots + ALU pipe (PRMT widening and the 3-input max); shared memory at about half its rate"
+        "limiter": ("ALU pipe (PRMT operand selection, DPX add-max and 3-input max: 96 % busy)" if cap is NCU_CAPTURES["scan_filter_lq_kernel_pssm"]
+                    else "issue slots + ALU pipe (PRMT widening and the 3-input max); shared memory at about half its rate"
                     if kernel == "scan_filter_lq_kernel" else "shared-memory wavefronts"),
         "limiter_source": cap["source"],
     }
