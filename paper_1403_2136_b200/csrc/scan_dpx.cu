@@ -511,6 +511,7 @@ cudaError_t launch_scan_two_pass(const mss_genome* g, const ScanParams& p0, void
         p.reads = p0.reads + (int64_t)c0 * p0.stride_words;
         p.reads_nmask = p0.reads_nmask ? p0.reads_nmask + (int64_t)c0 * ((p0.stride_words + 1) / 2) : nullptr;
         p.lens = p0.lens + c0;
+        p.pssm = p0.pssm ? p0.pssm + (int64_t)c0 * p0.pssm_stride : nullptr;       // the chunk's rows of the base-quality table
         p.ubound = nullptr;
         e = launch_scan_filter(g, p, ubound, st, &fgrid, &fsmem, &ftile, &frpb, &fkind);
         if (e != cudaSuccess) return e;

@@ -269,3 +269,24 @@ def test_pssm_takes_the_two_pass_scan(oracle_mod, tiny):
     _cmp(got, want, "pssm two-pass")
     _cmp(map_reads_pssm(G, reads, lens, d_pssm, strands=3, variant=13), want, "pssm, tile kernel requested")
     assert mss.mss_get_last_launch()["pass1_kernel"] == 0
+
+
+def test_pssm_two_pass_chunk_loop(oracle_mod, tiny):
+    """The two-pass scan works through the reads in chunks; every chunk must see ITS rows of the base-quality table (a chunk
+    that read the first rows again would still produce plausible records).  1, 7 and 100 reads per chunk."""
+    import paper_1403_2136_b200 as mss
+    from gpu_util import load_genome, map_reads_pssm, pssm_tables
+    cfg, g, reads, lens, quals = tiny
+    d_pssm, _, _ = pssm_tables(quals, lens)
+    wpm, wpmm = oracle_mod.pssm_from_phred(quals, 5, -4, 16)
+    want = oracle_mod.map_reads_pssm_parallel(g, cfg.frag_len, -1, reads, lens, wpm, wpmm, strands=3)
+    G = load_genome(g, cfg.frag_len, -1)
+    try:
+        for nbytes in (20_000, 1400, 200):                # 50 fragments x 2 strands x 2 B = 200 B of bounds per read
+            mss.mss_set_two_pass_chunk_bytes(nbytes)
+            got = map_reads_pssm(G, reads, lens, d_pssm, strands=3)
+            info = mss.mss_get_last_launch()
+            assert info["variant"] == 7 and info["launches"] >= 2 * (reads.shape[0] * 200 // nbytes)
+            _cmp(got, want, f"pssm chunk bytes {nbytes}")
+    finally:
+        mss.mss_set_two_pass_chunk_bytes(0)
