@@ -64,7 +64,8 @@ typedef enum {
     MSS_ERR_RANGE = -2,      /* match <= 0, mismatch >= 0, gap >= 0, max_len*match > 32767, mismatch < -32768,
                                 frag_len > 2^24, number of fragments > 2^31-1, max_len > MSS_MAX_READ_LEN */
     MSS_ERR_WORKSPACE = -3,  /* workspace_bytes smaller than the matching *_workspace_bytes query */
-    MSS_ERR_CUDA = -4        /* no device, launch failure, or any CUDA runtime error (see mss_last_cuda_error) */
+    MSS_ERR_CUDA = -4,       /* no device, launch failure, or any CUDA runtime error (see mss_last_cuda_error) */
+    MSS_ERR_STATIC_LIMIT = -5 /* mss_map_reads_static: the batch needs more scratch than MSS_STATIC_SCRATCH_BYTES */
 } mss_status;
 
 #define MSS_MAX_READ_LEN 6553   /* floor(32767 / 5): packed 16-bit score lanes stay exact; checked against match */
@@ -236,6 +237,30 @@ int mss_map_align_host(const mss_genome_t *g, const uint32_t *h_reads, const uin
 const char *mss_strerror(int status);
 int mss_last_cuda_error(void);                 /* cudaError_t of the last MSS_ERR_CUDA on this thread, 0 if none */
 int mss_version(void);                         /* 100*major + minor */
+
+/*
+ * mss_map_reads without a caller workspace, for callers that cannot allocate or hand over device scratch (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same inputs, same records, same kernels as
+ * mss_map_reads; the scan's scratch lives in a static device array of MSS_STATIC_SCRATCH_BYTES inside the
+ * library, which every GPU that loads the library holds until the process exits.  The call allocates nothing (no cudaMalloc,
+ * cudaFree or allocating library routine) and only enqueues work on `stream`.
+ *   limit      mss_map_workspace_bytes(g, n_reads, max_len, strands) <= MSS_STATIC_SCRATCH_BYTES, else MSS_ERR_STATIC_LIMIT
+ *              (nothing is launched): at the E. coli-sized geometry (1124 fragments, both strands) about 7,400 reads per call;
+ *              larger batches go through mss_map_reads, or in several calls.
+ *   sharing    every call on a device uses the SAME array, which keeps the previous call's contents.  Nothing in it has to start
+ *              at zero (every bound / partial record is written before it is read), so no clearing is needed -- but two calls
+ *              whose kernels overlap on the GPU (different streams, or concurrent graphs) race on it: serialise them.
+ *   set-up     mss_static_init(), once per device with that device current, resolves the array's device address
+ *              (cudaGetSymbolAddress; this is also where a lazily loaded module is brought in).  mss_map_reads_static does it
+ *              on first use if it was not called; callers that capture graphs call it before capture.
+ * Other errors as mss_map_reads.  mss_static_scratch_bytes() returns MSS_STATIC_SCRATCH_BYTES.
+ */
+#define MSS_STATIC_SCRATCH_BYTES (32u << 20)
+size_t mss_static_scratch_bytes(void);
+int mss_static_init(void);
+int mss_map_reads_static(const mss_genome_t *g, const uint32_t *d_reads, const uint32_t *d_reads_nmask,
+                         int32_t read_stride_words, const int32_t *d_lens, int32_t n_reads, int32_t max_len,
+                         mss_scoring_t sc, int32_t strands, void *stream, mss_top2_t *d_out);
 
 /*
  * Tuning / introspection (does not change results): select the scan kernel variant (0 = automatic: the two-pass scan

@@ -94,6 +94,9 @@ def lib() -> C.CDLL:
     L.mss_map_reads_pssm.restype = C.c_int
     L.mss_nw_align_pssm.argtypes = [vp, vp, vp, i32, vp, i32, i32, vp, vp, i32, _Scoring, i32, vp, sz, vp, vp, vp, vp, i32, vp]
     L.mss_nw_align_pssm.restype = C.c_int
+    L.mss_static_scratch_bytes.argtypes = []; L.mss_static_scratch_bytes.restype = C.c_size_t
+    L.mss_static_init.argtypes = []; L.mss_static_init.restype = C.c_int
+    L.mss_map_reads_static.argtypes = [vp, vp, vp, i32, vp, i32, i32, _Scoring, i32, vp, vp]; L.mss_map_reads_static.restype = C.c_int
     L.mss_strerror.argtypes = [C.c_int]; L.mss_strerror.restype = C.c_char_p
     L.mss_last_cuda_error.argtypes = []; L.mss_last_cuda_error.restype = C.c_int
     L.mss_version.argtypes = []; L.mss_version.restype = C.c_int
@@ -383,6 +386,29 @@ def mss_mapq_filter(d_hits, mapq_threshold: float = -1.0, stream=None):
     _check(lib().mss_mapq_filter(_ptr(d_hits), n, float(mapq_threshold), _stream(stream), _ptr(mapped), _ptr(mapq)),
            "mss_mapq_filter")
     return mapped, mapq
+
+
+MSS_ERR_STATIC_LIMIT = -5
+
+
+def mss_static_scratch_bytes() -> int:
+    return int(lib().mss_static_scratch_bytes())
+
+
+def mss_static_init() -> None:
+    """Resolve the static scratch array on the current device (once per device; before graph capture)."""
+    _check(lib().mss_static_init(), "mss_static_init")
+
+
+def mss_map_reads_static(g: Genome, d_reads, d_reads_nmask, d_lens, max_len: int, out, scoring: Scoring = Scoring(),
+                         strands: int = MSS_BOTH, stream=None):
+    """mss_map_reads into the caller's `out` (CUDA int32 tensor (n, 2, 4)) with the scan's scratch in the library's static
+    device array: the call allocates nothing.  Raises MssError(status MSS_ERR_STATIC_LIMIT) when the batch needs more scratch
+    than mss_static_scratch_bytes()."""
+    n = int(d_lens.numel())
+    _check(lib().mss_map_reads_static(g.handle, _ptr(d_reads), _ptr(d_reads_nmask), int(d_reads.shape[1]), _ptr(d_lens), n,
+                                      int(max_len), scoring.c(), strands, _stream(stream), _ptr(out)), "mss_map_reads_static")
+    return out
 
 
 def mss_set_two_pass_chunk_bytes(nbytes: int) -> None:

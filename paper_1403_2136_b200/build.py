@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmss.so")
-SOURCES = ["mss_api.cu", "genome.cu", "scan_generic.cu", "scan_dpx.cu", "scan_filter.cu", "scan_filter_lq.cu", "nw.cu", "aux.cu"]
+SOURCES = ["mss_api.cu", "genome.cu", "scan_generic.cu", "scan_dpx.cu", "scan_filter.cu", "scan_filter_lq.cu", "noalloc.cu", "nw.cu", "aux.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "--use_fast_math", "-Xptxas", "-v"]
 

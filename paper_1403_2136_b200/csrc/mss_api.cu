@@ -36,6 +36,8 @@ int check_scoring_scan(mss_scoring_t sc, int32_t max_len)
 }
 }  // namespace
 
+int mss_record_cuda_error(cudaError_t e) { return cuda_fail(e); }
+
 extern "C" {
 
 size_t mss_genome_workspace_bytes(int64_t n_bases, int32_t frag_len, int32_t overlap)
@@ -393,6 +395,7 @@ const char* mss_strerror(int status)
         case MSS_ERR_RANGE: return "value outside the supported range (scores, read length or fragment geometry)";
         case MSS_ERR_WORKSPACE: return "workspace too small";
         case MSS_ERR_CUDA: return "CUDA error (see mss_last_cuda_error)";
+        case MSS_ERR_STATIC_LIMIT: return "the request needs more scratch than the library's built-in static buffer (mss_static_scratch_bytes): use mss_map_reads with a caller workspace";
         default: return "unknown status";
     }
 }

@@ -91,6 +91,9 @@ __device__ __forceinline__ uint32_t read_base(const uint32_t* rw, const uint32_t
     return strand ? (3u - c) : c;
 }
 
+// records e for mss_last_cuda_error on this thread and returns MSS_ERR_CUDA (mss_api.cu)
+int mss_record_cuda_error(cudaError_t e);
+
 // launchers (each returns a cudaError_t)
 cudaError_t launch_genome_prepare(const uint32_t* d_packed, const uint32_t* d_nmask, int64_t n_bases,
                                   int64_t padded_bases, uint32_t* out_packed, uint32_t* out_nmask, cudaStream_t st);
