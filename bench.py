@@ -33,7 +33,7 @@ ISSUE_LANES_PER_CLK_SM = 128        # one warp instruction per clock per SM sub-
 SMEM_BYTES_PER_CLK_SM = 128         # shared-memory data pipe: one 128-byte wavefront per clock per SM
 # ncu --set full captures of the dominant kernels at ONE launch size (config 2, 4096 reads); quoted only for that launch
 NCU_CAPTURES = {
-    "scan_filter_lq_kernel": {"dram_bytes": 2_073_088, "instr_per_cell": 0.828, "smem_bytes_per_cell": 0.5,
+    "scan_filter_lq_kernel": {"dram_bytes": 2_115_840, "instr_per_cell": 0.814, "smem_bytes_per_cell": 0.5,
                               "source": "profiles/r2_scan_filter_lq_full.md"},
     "scan_filter_lq_kernel_pssm": {"dram_bytes": 3_751_424, "instr_per_cell": 1.044, "smem_bytes_per_cell": 1.0,
                                    "source": "profiles/r2_other_kernels.md"},

@@ -277,7 +277,8 @@ int mss_map_reads_static(const mss_genome_t *g, const uint32_t *d_reads, const u
 int mss_set_scan_variant(int variant);
 typedef struct {
     int32_t variant, grid, block, smem_bytes, reads_per_block, tile_diagonals, launches;
-    int32_t pass1_kernel;   /* two-pass scan: 1 = tile kernel, 2 / 3 / 4 = lane-per-query kernel with int16 DPX / fp16 / e5m2 operands; else 0 */
+    int32_t pass1_kernel;   /* two-pass scan: 1 = tile kernel, 2 / 3 / 4 = lane-per-query kernel with int16 DPX / fp16 / e5m2 operands and the
+                               plane offsets in registers, 6 / 7 / 8 = the same with the offsets in a shared-memory table, 5 = its PSSM form; else 0 */
 } mss_launch_info_t;
 int mss_get_last_launch(mss_launch_info_t *out);
 
@@ -298,7 +299,10 @@ int mss_set_two_pass_chunk_bytes(int64_t bytes);
  * take makes pass 1 fall back to the tile kernel.  arithmetic: how the chains are computed -- 0 = packed int16 DPX
  * (VIADDMNMX.S16x2.RELU), 1 = fp16 pairs (HFMA2.RELU; exact, every value is an integer <= 2048), 2 = e5m2 operand bytes
  * widened to fp16 pairs (half the shared-memory traffic), -1 = automatic: the highest of these the scoring and the read
- * length allow (a forced value that they do not allow is lowered the same way).  Bad values: MSS_ERR_ARG. */
+ * length allow (a forced value that they do not allow is lowered the same way).  Adding 8 (8..10, 11 = automatic arithmetic)
+ * makes the kernel read a query's plane offsets from its shared-memory table instead of registers, adding 16 (16..19) keeps
+ * them in registers where the read length allows (up to 256 scored positions); default: registers up to that length.
+ * Bad values: MSS_ERR_ARG. */
 int mss_set_pass1_geometry(int32_t query_sets, int32_t tile_window_starts, int32_t arithmetic);
 int mss_get_pass_times(float *h_pass1_ms, float *h_pass2_ms);
 

@@ -56,6 +56,10 @@ constexpr int LQ_NPL_N = 31;
 constexpr int LQ_ZERO_PLANE = 20;
 constexpr int LQ_MAX_QSETS = 4;
 enum { LQ_S16 = 0, LQ_F16 = 1, LQ_F8 = 2, LQ_PSSM = 3 };
+constexpr int LQ_TABLE = 8;         // host side: flag on the arithmetic = plane offsets from the shared-memory table
+#ifndef LQ_TABLE_FROM_NJ
+#define LQ_TABLE_FROM_NJ 80         // reads of more double steps than this (> 160 scored positions) take the table-driven instance
+#endif
 
 struct LqTile {
     int32_t HALF, ROWW, NG;         // tile = 2*HALF window starts; plane stride (words); column groups per warp and tile
@@ -99,17 +103,22 @@ __device__ __forceinline__ uint32_t lq_enc(int32_t v)            // one lane's o
     return (uint32_t)__half_as_ushort(__int2half_rn(v));
 }
 
-// NJ     = most double steps of a query this instantiation holds (even)
+// NJ     = most double steps of a query this instantiation holds in registers (even); 0 = none: the plane offsets of a
+//          query come from a shared-memory table, one 8-byte entry (two offsets) per pair of double steps, read by one
+//          LDS.64 per pair and shared by the thread's 8 chains (any read length the table leaves room for; no padding
+//          steps beyond the pair; ~50 registers fewer)
 // PACKED = two 16-bit word offsets per register (long reads) instead of one byte offset per register
 template <int NJ, bool PACKED, int MODE>
 __global__ void __launch_bounds__(32 * LQ_NW, LQ_BLOCKS_PER_SM)
 scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
 {
     constexpr int K = LQ_K, NW = LQ_NW, T = 32 * NW;
-    constexpr int NREG = PACKED ? NJ / 2 : NJ;
+    constexpr bool TABLE = (NJ == 0);
+    constexpr int NREG = TABLE ? 1 : (PACKED ? NJ / 2 : NJ);
     constexpr bool BYTEP = (MODE == LQ_F8 || MODE == LQ_PSSM);   // planes hold one byte per (column, window start): two columns per word
     // PSSM: a query's table of (operands, plane offset) per double step: ug.tstride 16-byte entries (odd: conflict-free LDS.128)
-    const int32_t TABW = (MODE == LQ_PSSM) ? 4 * ug.tstride : 0;
+    // TABLE: a query's table of offset pairs: ug.tstride 8-byte entries (odd: conflict-free LDS.64)
+    const int32_t TABW = (MODE == LQ_PSSM) ? 4 * ug.tstride : (TABLE ? 2 * ug.tstride : 0);
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t* wres = smem;                                      // NW * 32: per (warp, lane) tile maximum
     int32_t* qnj = (int32_t*)(wres + NW * 32);                  // 32 * qsets: double steps of a query; 0 = not scanned
@@ -176,7 +185,8 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
     const int32_t mystrand = (ns == 2) ? (myq & 1) : (p.strands == 2 ? 1 : 0);
     const uint32_t* myprow = (MODE == LQ_PSSM && myq < nq) ? p.pssm + (int64_t)(r0 + myq / ns) * p.pssm_stride : nullptr;
     uint4* mytab_w = reinterpret_cast<uint4*>(tab) + (size_t)myq * ug.tstride;
-    (void)mystrand; (void)myprow; (void)mytab_w;
+    uint2* mytab2 = reinterpret_cast<uint2*>(tab) + (size_t)myq * ug.tstride;
+    (void)mystrand; (void)myprow; (void)mytab_w; (void)mytab2;
     // word offset (plane, column) of the operand of double step j for chain 0 of group 0; padding steps: the zero plane
     auto step_word = [&](int32_t j) -> uint32_t {
         uint32_t plane = LQ_ZERO_PLANE, col = 0u;
@@ -188,11 +198,15 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
             else plane = b2 < 4u ? 25u + b2 : (b2 == 5u ? 30u : 29u);
             col = (uint32_t)i1;
         }
-        const uint32_t cw = col + (MODE == LQ_PSSM ? 0u : (uint32_t)(ws * CW));     // column of chain 0, group 0 (PSSM: of warp 0)
+        const uint32_t cw = col + ((MODE == LQ_PSSM || TABLE) ? 0u : (uint32_t)(ws * CW));     // column of chain 0, group 0 (tables: of warp 0)
         return plane * (uint32_t)ROWW + (BYTEP ? cw >> 1 : cw);
     };
     uint32_t off[NREG];
-    if (MODE != LQ_PSSM) {
+    if (TABLE && MODE != LQ_PSSM) {
+        // written by the first warp of the query's set, shared by the others (whose column share goes into the group base)
+        for (int32_t jp = 0; jp < (ws == 0 ? ug.tstride : 0); jp++)
+            mytab2[jp] = make_uint2(step_word(2 * jp) * 4u, step_word(2 * jp + 1) * 4u);
+    } else if (MODE != LQ_PSSM) {
 #pragma unroll
         for (int j = 0; j < NJ; j++) {
             const uint32_t w = step_word(j);
@@ -362,7 +376,8 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
             // ---- a3: this lane's query against the warp's columns of the tile --------------------------------------
             uint32_t tmax = 0u;
             for (int32_t g = 0; g < tg.NG; g++) {
-                const char* pg = planes_b + g * (BYTEP ? K * 2 : K * 4) + (MODE == LQ_PSSM ? ws * CW * 2 : 0);   // warp-uniform group base
+                const char* pg = planes_b + g * (BYTEP ? K * 2 : K * 4)
+                               + ((MODE == LQ_PSSM || TABLE) ? ws * CW * (BYTEP ? 2 : 4) : 0);   // warp-uniform group base
                 uint32_t H[K], B[K];
 #pragma unroll
                 for (int k = 0; k < K; k++) { H[k] = 0u; B[k] = 0u; }
@@ -422,6 +437,12 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                         const uint4 ta = mytab[j], tb = mytab[j + 1];
                         pair(ta.z, tb.z, make_uint4(ta.x, ta.y, tb.x, tb.y));
                     }
+                } else if (TABLE) {
+#pragma unroll 4
+                    for (int32_t jp = 0; jp < (njb >> 1); jp++) {
+                        const uint2 o = mytab2[jp];
+                        pair(o.x, o.y, make_uint4(0u, 0u, 0u, 0u));
+                    }
                 } else {
 #pragma unroll
                     for (int j = 0; j < NJ; j += 2) {
@@ -473,8 +494,15 @@ int32_t lq_tstride(int32_t max_len, int32_t istep)
     int32_t steps = (max_len + istep - 1) / istep;
     return ((((steps + 1) / 2) + 1) & ~1) | 1;
 }
-LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode, int npl, int32_t qsets)
+// TABLE: entries (pairs of double steps) per query, made odd
+int32_t lq_pstride(int32_t max_len, int32_t istep)
 {
+    int32_t steps = (max_len + istep - 1) / istep;
+    return ((((steps + 1) / 2) + 1) / 2) | 1;
+}
+LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int modef, int npl, int32_t qsets)
+{
+    const int mode = modef & 7;
     // columns read: chain column < HALF, plus the column of the last double step (< max_len rounded up to even steps)
     LqSmem s;
     int32_t halo = ((max_len + 2 * istep + 3) & ~3);
@@ -487,6 +515,7 @@ LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode, int npl, 
     // planes, wres, qnj + qm, raw words (2 buffers), raw mask words (2 buffers), pad to 16 bytes, codes
     size_t words = (size_t)npl * roww + LQ_NW * 32 + 2 * 32 * LQ_MAX_QSETS + 2 * s.NRAW + 2 * (s.NRAW / 2 + 1);
     if (mode == LQ_PSSM) words += (size_t)32 * qsets * 4 * lq_tstride(max_len, istep);     // per-query (operands, offset) tables
+    else if (modef & LQ_TABLE) words += (size_t)32 * qsets * 2 * lq_pstride(max_len, istep);   // per-query offset-pair tables
     words = (words + 3) & ~(size_t)3;
     s.bytes = words * 4 + (size_t)16 * s.NRAW;
     return s;
@@ -495,6 +524,7 @@ LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int mode, int npl, 
 thread_local int t_lq_qsets = 0;       // tuning hook: query sets per block (reads per block = 16 * qsets with both strands); 0 = by batch size
 thread_local int t_lq_half = 0;        // tuning hook: force the tile (0 = automatic)
 thread_local int t_lq_mode = -1;       // tuning hook: force the arithmetic (-1 = automatic)
+thread_local int t_lq_table = -1;      // tuning hook: plane offsets from the shared-memory table (1), in registers (0), automatic (-1)
 
 int lq_mode(const ScanParams& p)
 {
@@ -507,6 +537,24 @@ int lq_mode(const ScanParams& p)
     if (want == LQ_F8 && !f8_ok) want = LQ_F16;
     if (want == LQ_F16 && !f16_ok) want = LQ_S16;
     return want;
+}
+
+int32_t lq_double_steps(const ScanParams& p);
+
+// arithmetic | LQ_TABLE: where a query's plane offsets live.  Registers hold at most 128 double steps (256 scored positions);
+// beyond that, and where it measured faster, they come from the shared-memory table.  Measured (e5m2 operands, cells/clk/SM,
+// registers / table): 36 bp 129.8 / 118.2, 100 bp 136.7 / 124.5, 150 bp 124.6 / 124.2, 250 bp 112.1 (16-bit offset pairs) /
+// 126.5: the table costs one LDS.64 per pair of double steps and a rolled loop, and is the same for every length.
+int lq_plan(const ScanParams& p)
+{
+    const int mode = lq_mode(p);
+    if (mode == LQ_PSSM) return mode;
+    const int32_t nj = lq_double_steps(p);
+    bool table = nj > LQ_TABLE_FROM_NJ;
+    if (t_lq_table == 1) table = true;
+    if (t_lq_table == 0 && nj <= 128) table = false;
+    if (nj > 128) table = true;
+    return mode | (table ? LQ_TABLE : 0);
 }
 
 // the tile: 2*HALF window starts, HALF a multiple of the columns one more group of every warp of a set adds;
@@ -542,19 +590,26 @@ bool lq_pick(const mss_genome* g, const ScanParams& p, int32_t qsets, int mode, 
     size_t ba = 0, bb = 0;
     if (!lq_pick_tile(g, p, qsets, mode, LQ_NPL, t_lq_half, &a, &ba)) return false;
     if (!lq_pick_tile(g, p, qsets, mode, LQ_NPL_N, 0, &b, &bb)) { b = LqTile{0, 0, 0, 0, 0}; bb = 0; }
-    if (out) { out->a = a; out->b = b; out->qsets = qsets; out->tstride = lq_tstride(p.max_len, p.istep); }
+    if (out) { out->a = a; out->b = b; out->qsets = qsets; out->tstride = (mode & LQ_TABLE) ? lq_pstride(p.max_len, p.istep) : lq_tstride(p.max_len, p.istep); }
     if (bytes) *bytes = ba > bb ? ba : bb;
     return true;
 }
 
-// query sets per block: more sets amortise the tile staging over more queries (measured on config 2: 131.0 / 133.0 / 133.8
-// cells/clk/SM with 1 / 2 / 4 sets), fewer keep the grid fine for small batches
-int32_t lq_qsets(const ScanParams& p)
+// query sets per block: more sets amortise the tile staging over more queries (measured, cells/clk/SM with 1 / 2 / 4 sets:
+// 133.4 / 135.5 / 136.8 at 100 bp, 121.5 / 126.6 / 129.8 at 36 bp, 122.2 / 123.6 / 124.5 at 150 bp): the most sets with which
+// the grid (read groups x fragments) still fills the GPU's ~48 waves of resident blocks
+int32_t lq_qsets(const mss_genome* g, const ScanParams& p)
 {
     if (p.pssm) return 1;                                       // the per-query tables take the room more query sets would need
     if (t_lq_qsets) return t_lq_qsets;
+    int32_t most = 4;                                           // offset tables: at most 40 kB of them beside the tile
+    if (lq_plan(p) & LQ_TABLE)
+        while (most > 1 && (size_t)32 * most * 8 * lq_pstride(p.max_len, p.istep) > 40960) most >>= 1;
     const int64_t queries = (int64_t)p.n_reads * (p.strands == 3 ? 2 : 1);
-    return queries >= 65536 ? 4 : (queries >= 16384 ? 2 : 1);
+    const int64_t target = (int64_t)g->sm_count * LQ_BLOCKS_PER_SM * 48;
+    for (int32_t qs = most; qs > 1; qs >>= 1)
+        if (((queries + 32 * qs - 1) / (32 * qs)) * (int64_t)g->n_frag >= target) return qs;
+    return 1;
 }
 
 // the kernel instance (most double steps held) that serves queries of up to nj double steps
@@ -602,24 +657,26 @@ void scan_filter_lq_tune(int qsets, int half, int mode)
 {
     t_lq_qsets = (qsets == 1 || qsets == 2 || qsets == 4) ? qsets : 0;
     t_lq_half = half > 0 ? half : 0;
+    // mode: -1 automatic; 0..2 the arithmetic; + 8 = offsets from the table, + 16 = offsets in registers (3 = automatic arithmetic)
+    t_lq_table = -1;
+    if (mode >= 16) { t_lq_table = 0; mode -= 16; } else if (mode >= 8) { t_lq_table = 1; mode -= 8; }
     t_lq_mode = (mode >= 0 && mode <= 2) ? mode : -1;
 }
 
 bool scan_filter_lq_supported(const mss_genome* g, const ScanParams& p)
 {
     if (p.pssm && p.istep != 1) return false;
-    if (lq_double_steps(p) > 128) return false;                 // longer queries: the tile kernel of scan_filter.cu
-    return lq_pick(g, p, lq_qsets(p), lq_mode(p), nullptr, nullptr);
+    return lq_pick(g, p, lq_qsets(g, p), lq_plan(p), nullptr, nullptr);      // no tile fits (very long reads): the tile kernel of scan_filter.cu
 }
 
 cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint16_t* ubound, cudaStream_t st, int32_t* grid_out,
                                   int32_t* smem_out, int32_t* tile_out, int32_t* rpb_out, int32_t* kind_out)
 {
     LqGeom ug;
-    const int mode = lq_mode(p);
-    if (kind_out) *kind_out = 2 + mode;
+    const int plan = lq_plan(p), mode = plan & 7;
+    if (kind_out) *kind_out = ((plan & LQ_TABLE) ? 6 : 2) + mode;
     size_t smem = 0;
-    if (!lq_pick(g, p, lq_qsets(p), mode, &ug, &smem)) return cudaErrorInvalidConfiguration;
+    if (!lq_pick(g, p, lq_qsets(g, p), plan, &ug, &smem)) return cudaErrorInvalidConfiguration;
     const int32_t ns = p.strands == 3 ? 2 : 1;
     ug.reads_per_group = 32 * ug.qsets / ns;
     ug.n_groups = (p.n_reads + ug.reads_per_group - 1) / ug.reads_per_group;
@@ -637,6 +694,7 @@ cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint
     // padding steps cost time (the early-exit check is coarse): the common read lengths get a tight instance of the
     // fast arithmetic (36, 51, 76, 100 bp)
     if (mode == LQ_PSSM) return lq_launch3<2, false, LQ_PSSM>(p, ug, ubound, st, smem);   // table-driven: one instance for every length
+    if (plan & LQ_TABLE) return lq_launch<0, false>(mode, p, ug, ubound, st, smem);
     switch (lq_nj_instance(lq_double_steps(p), mode)) {
         case 18: return lq_launch3<18, false, LQ_F8>(p, ug, ubound, st, smem);
         case 26: return lq_launch3<26, false, LQ_F8>(p, ug, ubound, st, smem);

@@ -18,7 +18,8 @@ def _cmp(got, want, ctx=""):
 # pass-1 kernels and arithmetic: (scan variant, arithmetic of the lane-per-query kernel)
 #   (7, -1) automatic = lane-per-query kernel, e5m2 operand bytes where the scoring allows; (7, 0) packed int16 DPX;
 #   (7, 1) fp16 pairs; (7, 2) e5m2 bytes (lowered where the scoring is not exact in e5m2); (13, -1) the tile kernel
-PASS1 = [(7, -1), (7, 0), (7, 1), (7, 2), (13, -1)]
+#   (7, 8) / (7, 10) int16 / e5m2 arithmetic with the plane offsets read from the shared-memory table instead of registers
+PASS1 = [(7, -1), (7, 0), (7, 1), (7, 2), (7, 8), (7, 10), (13, -1)]
 
 
 class pass1_setup:
@@ -158,11 +159,12 @@ def test_two_pass_records_equal_oracle(oracle_mod, F, V, strands):
                  f"two-pass fast {variant}/{arith} F={F} V={V} strands={strands}")
 
 
-@pytest.mark.parametrize("m", [1, 2, 3, 35, 64, 127, 128, 129, 159, 160, 161, 255, 256, 257, 300])
+@pytest.mark.parametrize("m", [1, 2, 3, 35, 64, 127, 128, 129, 159, 160, 161, 255, 256, 257, 300, 409, 600])
 def test_two_pass_read_lengths_across_the_register_table_limits(oracle_mod, m):
     """The lane-per-query pass 1 keeps a query's plane offsets in registers: 32, 64 or 80 double steps directly, up to 128
-    as 16-bit pairs; longer reads take the tile kernel.  Lengths on both sides of every limit, mixed with shorter reads in
-    the same block (padding steps on the all-zero plane), all three arithmetics."""
+    as 16-bit pairs; longer reads read them from the shared-memory table (and the longest take the tile kernel).  Lengths on
+    both sides of every limit, mixed with shorter reads in the same block (padding steps on the all-zero plane), all three
+    arithmetics, offsets in registers and from the table."""
     from gpu_util import load_genome, map_reads
     g = gen.make_genome(30_000, 36)[0]
     r = gen.make_reads(g, 40, m, 3600 + m, sub_rate=0.12, indel_prob=0.0 if m < 8 else 0.5)
@@ -172,7 +174,7 @@ def test_two_pass_read_lengths_across_the_register_table_limits(oracle_mod, m):
             lens[k] = short; reads[k, short:] = gen.N
     G = load_genome(g, 1536, -1)
     want = oracle_mod.map_reads_parallel(g, 1536, -1, reads, lens, strands=3)
-    for arith in (0, 1, 2):
+    for arith in (0, 1, 2, 8, 9, 10):
         with pass1_setup(7, arith):
             _cmp(map_reads(G, reads, lens, strands=3, variant=7), want, f"m={m} arithmetic {arith}")
 
