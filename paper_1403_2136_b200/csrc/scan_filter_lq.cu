@@ -621,6 +621,7 @@ int32_t lq_nj_instance(int32_t nj, int mode)
         if (nj > 32 && nj <= 38) return 38;
     }
     if (mode == LQ_F8 && nj > 38 && nj <= 50) return 50;
+    if (mode == LQ_F8 && nj > 64 && nj <= 76) return 76;
     if (nj <= 32) return 32;
     if (nj <= 64) return 64;
     if (nj <= 80) return 80;
@@ -692,7 +693,7 @@ cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint
     if (tile_out) *tile_out = 2 * ug.a.HALF;
     if (rpb_out) *rpb_out = ug.reads_per_group;
     // padding steps cost time (the early-exit check is coarse): the common read lengths get a tight instance of the
-    // fast arithmetic (36, 51, 76, 100 bp)
+    // fast arithmetic (36, 51, 76, 100, 150 bp)
     if (mode == LQ_PSSM) return lq_launch3<2, false, LQ_PSSM>(p, ug, ubound, st, smem);   // table-driven: one instance for every length
     if (plan & LQ_TABLE) return lq_launch<0, false>(mode, p, ug, ubound, st, smem);
     switch (lq_nj_instance(lq_double_steps(p), mode)) {
@@ -700,6 +701,7 @@ cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint
         case 26: return lq_launch3<26, false, LQ_F8>(p, ug, ubound, st, smem);
         case 38: return lq_launch3<38, false, LQ_F8>(p, ug, ubound, st, smem);
         case 50: return lq_launch3<50, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 76: return lq_launch3<76, false, LQ_F8>(p, ug, ubound, st, smem);
         case 32: return lq_launch<32, false>(mode, p, ug, ubound, st, smem);
         case 64: return lq_launch<64, false>(mode, p, ug, ubound, st, smem);
         case 80: return lq_launch<80, false>(mode, p, ug, ubound, st, smem);
