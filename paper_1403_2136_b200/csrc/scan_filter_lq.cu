@@ -543,7 +543,7 @@ int32_t lq_double_steps(const ScanParams& p);
 
 // arithmetic | LQ_TABLE: where a query's plane offsets live.  Registers hold at most 128 double steps (256 scored positions);
 // beyond that, and where it measured faster, they come from the shared-memory table.  Measured (e5m2 operands, cells/clk/SM,
-// registers / table): 36 bp 129.8 / 118.2, 100 bp 136.7 / 124.5, 150 bp 124.6 / 124.2, 250 bp 112.1 (16-bit offset pairs) /
+// registers / table): 36 bp 129.8 / 118.2, 100 bp 136.7 / 124.5, 150 bp 133.1 / 125.3, 250 bp 112.1 (16-bit offset pairs) /
 // 126.5: the table costs one LDS.64 per pair of double steps and a rolled loop, and is the same for every length.
 int lq_plan(const ScanParams& p)
 {
