@@ -467,7 +467,7 @@ scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
                     }
                 }
 #pragma unroll
-                for (int k = 0; k < K; k++) tmax = __vmaxs2(tmax, B[k]);
+                for (int k = 0; k < K; k += 2) tmax = __vimax3_s16x2(tmax, B[k], B[k + 1]);
             }
             wres[warp * 32 + lane] = max(tmax & 0xFFFFu, tmax >> 16);
             prev_f = f; prev_last = (tile == tiles_per_frag - 1);
