@@ -48,6 +48,20 @@ def test_host_side_argument_checks(L):
     assert L.mss_genome_free(None) == -1
 
 
+def test_tuning_switches_and_static_entry_point_check_their_arguments(L):
+    """Host-only: the round-2 additions reject bad values before touching a device."""
+    assert L.mss_set_scan_variant(13) == 0 and L.mss_set_scan_variant(14) == -1 and L.mss_set_scan_variant(0) == 0
+    for q, t, a, want in ((0, 0, -1, 0), (4, 4096, 2, 0), (2, 1024, 10, 0), (1, 0, 16, 0), (3, 0, -1, -1), (1, 1023, -1, -1),
+                          (1, -2, -1, -1), (1, 0, 3, -1), (1, 0, 12, -1), (1, 0, 20, -1), (1, 0, -2, -1), (0, 0, -1, 0)):
+        assert L.mss_set_pass1_geometry(q, t, a) == want, (q, t, a)
+    assert L.mss_set_two_pass_chunk_bytes(12345) == 0 and L.mss_set_two_pass_chunk_bytes(0) == 0
+    assert L.mss_static_scratch_bytes() == 32 << 20
+    assert b"static" in L.mss_strerror(-5)
+    sc = _Scoring(5, -4, -26)
+    assert L.mss_map_reads_static(None, None, None, 7, None, 10, 100, sc, 3, None, None) == -1
+    assert L.mss_map_reads_bounds_pssm(None, None, None, 7, None, 10, 100, None, 100, sc, 3, None, None, None) == -1
+
+
 def test_product_does_not_import_the_oracle():
     import os
     import re
