@@ -245,7 +245,8 @@ int mss_version(void);                         /* 100*major + minor */
  * library, which every GPU that loads the library holds until the process exits.  The call allocates nothing (no cudaMalloc,
  * cudaFree or allocating library routine) and only enqueues work on `stream`.
  *   limit      mss_map_workspace_bytes(g, n_reads, max_len, strands) <= MSS_STATIC_SCRATCH_BYTES, else MSS_ERR_STATIC_LIMIT
- *              (nothing is launched): at the E. coli-sized geometry (1124 fragments, both strands) about 7,400 reads per call;
+ *              (nothing is launched): at the E. coli-sized geometry (1124 fragments, both strands) about 3,700 reads per call
+ *              (the query is the maximum over every scan path: 8 B per read and fragment for the generic kernel);
  *              larger batches go through mss_map_reads, or in several calls.
  *   sharing    every call on a device uses the SAME array, which keeps the previous call's contents.  Nothing in it has to start
  *              at zero (every bound / partial record is written before it is read), so no clearing is needed -- but two calls
