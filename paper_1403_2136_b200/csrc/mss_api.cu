@@ -419,7 +419,7 @@ int mss_set_pass1_geometry(int32_t query_sets, int32_t tile_window_starts, int32
     if (!(query_sets == 0 || query_sets == 1 || query_sets == 2 || query_sets == 4)) return MSS_ERR_ARG;
     if (tile_window_starts < 0 || (tile_window_starts & 1)) return MSS_ERR_ARG;
     if (!(arithmetic == -1 || (arithmetic >= 0 && arithmetic <= 2) || (arithmetic >= 8 && arithmetic <= 11) ||
-          (arithmetic >= 16 && arithmetic <= 19))) return MSS_ERR_ARG;
+          (arithmetic >= 16 && arithmetic <= 19) || (arithmetic >= 32 && arithmetic <= 35))) return MSS_ERR_ARG;
     scan_filter_lq_tune(query_sets, tile_window_starts / 2, arithmetic);
     return MSS_OK;
 }

@@ -57,6 +57,10 @@ constexpr int LQ_ZERO_PLANE = 20;
 constexpr int LQ_MAX_QSETS = 4;
 enum { LQ_S16 = 0, LQ_F16 = 1, LQ_F8 = 2, LQ_PSSM = 3 };
 constexpr int LQ_TABLE = 8;         // host side: flag on the arithmetic = plane offsets from the shared-memory table
+constexpr int LQ_K16 = 16;          // host side: flag = the 16-chain instances (short reads)
+#ifndef LQ_K16_UP_TO_NJ
+#define LQ_K16_UP_TO_NJ 38          // reads of at most this many double steps (76 scored positions) take the 16-chain instances
+#endif
 #ifndef LQ_TABLE_FROM_NJ
 #define LQ_TABLE_FROM_NJ 80         // reads of more double steps than this (> 160 scored positions) take the table-driven instance
 #endif
@@ -108,11 +112,13 @@ __device__ __forceinline__ uint32_t lq_enc(int32_t v)            // one lane's o
 //          LDS.64 per pair and shared by the thread's 8 chains (any read length the table leaves room for; no padding
 //          steps beyond the pair; ~50 registers fewer)
 // PACKED = two 16-bit word offsets per register (long reads) instead of one byte offset per register
-template <int NJ, bool PACKED, int MODE>
+// KC     = chains per thread and column group (8; 16 for the short-read instances, whose few offset registers leave room: the
+//          per-group start-up and the per-double-step address are shared by twice as many cells)
+template <int NJ, bool PACKED, int MODE, int KC = LQ_K>
 __global__ void __launch_bounds__(32 * LQ_NW, LQ_BLOCKS_PER_SM)
 scan_filter_lq_kernel(ScanParams p, LqGeom ug, uint16_t* __restrict__ ubound)
 {
-    constexpr int K = LQ_K, NW = LQ_NW, T = 32 * NW;
+    constexpr int K = KC, NW = LQ_NW, T = 32 * NW;
     constexpr bool TABLE = (NJ == 0);
     constexpr int NREG = TABLE ? 1 : (PACKED ? NJ / 2 : NJ);
     constexpr bool BYTEP = (MODE == LQ_F8 || MODE == LQ_PSSM);   // planes hold one byte per (column, window start): two columns per word
@@ -524,6 +530,7 @@ LqSmem lq_smem(int32_t half, int32_t max_len, int32_t istep, int modef, int npl,
 thread_local int t_lq_qsets = 0;       // tuning hook: query sets per block (reads per block = 16 * qsets with both strands); 0 = by batch size
 thread_local int t_lq_half = 0;        // tuning hook: force the tile (0 = automatic)
 thread_local int t_lq_mode = -1;       // tuning hook: force the arithmetic (-1 = automatic)
+thread_local bool t_lq_k8 = false;     // tuning hook: 8 chains per thread even for short reads
 thread_local int t_lq_table = -1;      // tuning hook: plane offsets from the shared-memory table (1), in registers (0), automatic (-1)
 
 int lq_mode(const ScanParams& p)
@@ -540,6 +547,7 @@ int lq_mode(const ScanParams& p)
 }
 
 int32_t lq_double_steps(const ScanParams& p);
+int32_t lq_nj_instance(int32_t nj, int mode);
 
 // arithmetic | LQ_TABLE: where a query's plane offsets live.  Registers hold at most 128 double steps (256 scored positions);
 // beyond that, and where it measured faster, they come from the shared-memory table.  Measured (e5m2 operands, cells/clk/SM,
@@ -554,14 +562,16 @@ int lq_plan(const ScanParams& p)
     if (t_lq_table == 1) table = true;
     if (t_lq_table == 0 && nj <= 128) table = false;
     if (nj > 128) table = true;
-    return mode | (table ? LQ_TABLE : 0);
+    const int32_t inst = lq_nj_instance(nj, mode);              // only the tight short-read instances exist with 16 chains
+    const bool k16 = !table && mode == LQ_F8 && nj <= LQ_K16_UP_TO_NJ && (inst == 18 || inst == 26 || inst == 38) && !t_lq_k8;
+    return mode | (table ? LQ_TABLE : 0) | (k16 ? LQ_K16 : 0);
 }
 
 // the tile: 2*HALF window starts, HALF a multiple of the columns one more group of every warp of a set adds;
 // least padding of the fragment length first, larger tiles on ties; two blocks per SM must fit
 bool lq_pick_tile(const mss_genome* g, const ScanParams& p, int32_t qsets, int mode, int npl, int32_t forced_half, LqTile* out, size_t* bytes)
 {
-    const int32_t unit = (LQ_NW / qsets) * LQ_K;
+    const int32_t unit = (LQ_NW / qsets) * ((mode & LQ_K16) ? 16 : LQ_K);
     const size_t prologue = (size_t)32 * qsets * ((p.max_len + 3) & ~3);
     int32_t best = 0; double best_waste = 1e30;
     for (int32_t half = unit; half <= 4096; half += unit) {
@@ -634,13 +644,13 @@ int32_t lq_double_steps(const ScanParams& p)
     return (steps + 1) / 2;
 }
 
-template <int NJ, bool PACKED, int MODE>
+template <int NJ, bool PACKED, int MODE, int KC = LQ_K>
 cudaError_t lq_launch3(const ScanParams& p, const LqGeom& ug, uint16_t* ubound, cudaStream_t st, size_t smem)
 {
-    cudaError_t e = cudaFuncSetAttribute(scan_filter_lq_kernel<NJ, PACKED, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(scan_filter_lq_kernel<NJ, PACKED, MODE, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int64_t blocks = (int64_t)ug.n_groups * ug.n_splits;
-    scan_filter_lq_kernel<NJ, PACKED, MODE><<<(unsigned)blocks, 32 * LQ_NW, smem, st>>>(p, ug, ubound);
+    scan_filter_lq_kernel<NJ, PACKED, MODE, KC><<<(unsigned)blocks, 32 * LQ_NW, smem, st>>>(p, ug, ubound);
     return cudaGetLastError();
 }
 
@@ -659,7 +669,8 @@ void scan_filter_lq_tune(int qsets, int half, int mode)
     t_lq_qsets = (qsets == 1 || qsets == 2 || qsets == 4) ? qsets : 0;
     t_lq_half = half > 0 ? half : 0;
     // mode: -1 automatic; 0..2 the arithmetic; + 8 = offsets from the table, + 16 = offsets in registers (3 = automatic arithmetic)
-    t_lq_table = -1;
+    t_lq_table = -1; t_lq_k8 = false;
+    if (mode >= 32) { t_lq_k8 = true; mode -= 32; if (mode == 3) mode = -1; }
     if (mode >= 16) { t_lq_table = 0; mode -= 16; } else if (mode >= 8) { t_lq_table = 1; mode -= 8; }
     t_lq_mode = (mode >= 0 && mode <= 2) ? mode : -1;
 }
@@ -697,10 +708,10 @@ cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint
     if (mode == LQ_PSSM) return lq_launch3<2, false, LQ_PSSM>(p, ug, ubound, st, smem);   // table-driven: one instance for every length
     if (plan & LQ_TABLE) return lq_launch<0, false>(mode, p, ug, ubound, st, smem);
     switch (lq_nj_instance(lq_double_steps(p), mode)) {
-        case 18: return lq_launch3<18, false, LQ_F8>(p, ug, ubound, st, smem);
-        case 26: return lq_launch3<26, false, LQ_F8>(p, ug, ubound, st, smem);
-        case 38: return lq_launch3<38, false, LQ_F8>(p, ug, ubound, st, smem);
-        case 50: return lq_launch3<50, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 18: return (plan & LQ_K16) ? lq_launch3<18, false, LQ_F8, 16>(p, ug, ubound, st, smem) : lq_launch3<18, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 26: return (plan & LQ_K16) ? lq_launch3<26, false, LQ_F8, 16>(p, ug, ubound, st, smem) : lq_launch3<26, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 38: return (plan & LQ_K16) ? lq_launch3<38, false, LQ_F8, 16>(p, ug, ubound, st, smem) : lq_launch3<38, false, LQ_F8>(p, ug, ubound, st, smem);
+        case 50: return lq_launch3<50, false, LQ_F8>(p, ug, ubound, st, smem);     // 16 chains measured slower here (135.3 against 136.7)
         case 76: return lq_launch3<76, false, LQ_F8>(p, ug, ubound, st, smem);
         case 32: return lq_launch<32, false>(mode, p, ug, ubound, st, smem);
         case 64: return lq_launch<64, false>(mode, p, ug, ubound, st, smem);

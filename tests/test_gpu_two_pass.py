@@ -159,12 +159,14 @@ def test_two_pass_records_equal_oracle(oracle_mod, F, V, strands):
                  f"two-pass fast {variant}/{arith} F={F} V={V} strands={strands}")
 
 
-@pytest.mark.parametrize("m", [1, 2, 3, 35, 64, 127, 128, 129, 159, 160, 161, 255, 256, 257, 300, 409, 600])
+@pytest.mark.parametrize("m", [1, 2, 3, 35, 36, 37, 52, 53, 60, 64, 65, 76, 77, 100, 101, 127, 128, 129, 152, 153, 159, 160, 161, 255, 256, 257,
+                               300, 409, 600])
 def test_two_pass_read_lengths_across_the_register_table_limits(oracle_mod, m):
     """The lane-per-query pass 1 keeps a query's plane offsets in registers: 32, 64 or 80 double steps directly, up to 128
     as 16-bit pairs; longer reads read them from the shared-memory table (and the longest take the tile kernel).  Lengths on
     both sides of every limit, mixed with shorter reads in the same block (padding steps on the all-zero plane), all three
-    arithmetics, offsets in registers and from the table."""
+    arithmetics, offsets in registers and from the table, 8 and 16 chains per thread (the 16-chain instances serve 1-52 and
+    65-76 scored positions: lengths on both sides of those limits too)."""
     from gpu_util import load_genome, map_reads
     g = gen.make_genome(30_000, 36)[0]
     r = gen.make_reads(g, 40, m, 3600 + m, sub_rate=0.12, indel_prob=0.0 if m < 8 else 0.5)
@@ -174,7 +176,7 @@ def test_two_pass_read_lengths_across_the_register_table_limits(oracle_mod, m):
             lens[k] = short; reads[k, short:] = gen.N
     G = load_genome(g, 1536, -1)
     want = oracle_mod.map_reads_parallel(g, 1536, -1, reads, lens, strands=3)
-    for arith in (0, 1, 2, 8, 9, 10):
+    for arith in (-1, 0, 1, 2, 8, 9, 10, 34):
         with pass1_setup(7, arith):
             _cmp(map_reads(G, reads, lens, strands=3, variant=7), want, f"m={m} arithmetic {arith}")
 
