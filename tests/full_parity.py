@@ -31,6 +31,8 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--reads", type=int, default=None, help="first N reads of every group (default: all)")
     ap.add_argument("--mode", default="plain", choices=["plain", "fast", "pssm"])
+    ap.add_argument("--read-len", type=int, default=None,
+                    help="keep only the reads of this length (config 3: one length of the sweep per call, as bench.py --read-len does)")
     ap.add_argument("--nw-reads", type=int, default=4096, help="reads whose second stage is also compared (evenly spaced)")
     ap.add_argument("--skip", type=int, default=0, help="compare only reads [skip, n) with the oracle (the GPU still maps all)")
     ap.add_argument("--stop", type=int, default=None, help="compare only reads [skip, stop) (one gpurun call lasts at most an hour)")
@@ -47,6 +49,12 @@ def main():
     genome, _ = cfg.genome()
     r = cfg.reads(genome, limit=args.reads)
     reads, lens = r["reads"], r["lens"]
+    if args.read_len is not None:
+        keep = lens == args.read_len
+        reads, lens = np.ascontiguousarray(reads[keep][:, :args.read_len]), np.ascontiguousarray(lens[keep])
+        r = {k: (v[keep] if hasattr(v, "shape") and v.shape[:1] == keep.shape else v) for k, v in r.items()}
+        if lens.size == 0:
+            raise SystemExit(f"config {cfg.c} has no reads of length {args.read_len}")
     n, m = reads.shape
     dev = torch.device("cuda", 0)
     packed, nmask = gen.pack_2bit(genome)
@@ -121,7 +129,7 @@ def main():
     cells = float(np.sum(scored)) * per_frag                               # cells of the whole batch (what the GPU mapped)
     cells_compared = float(np.sum(scored[args.skip:stop])) * per_frag      # cells of the slice the oracle re-computed
     summary = {
-        "config": cfg.c, "name": cfg.name, "mode": args.mode, "reads": int(n), "read_len_max": int(m), "n_frag": int(G.n_frag),
+        "config": cfg.c, "name": cfg.name, "mode": args.mode, "read_len_filter": args.read_len, "reads": int(n), "read_len_max": int(m), "n_frag": int(G.n_frag),
         "cells": cells, "top2_compared": int(checked - args.skip), "first_read_compared": int(args.skip), "top2_mismatches": len(bad_top2), "first_bad_top2": bad_top2[:5],
         "nw_compared": int(len(idx)), "nw_mismatches": len(bad_nw), "first_bad_nw": bad_nw[:5],
         "ties_best_eq_second": int(np.sum(got[:, 0, 2] == got[:, 1, 2])),
