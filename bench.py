@@ -418,6 +418,10 @@ def main():
                     else "issue slots + ALU pipe (PRMT widening and the 3-input max); shared memory at about half its rate"
                     if kernel == "scan_filter_lq_kernel" else "shared-memory wavefronts"),
         "limiter_source": cap["source"],
+        "note": ("frac counts the algorithmic 0.375 instr/cell against the ALU/DPX pipe alone (BASELINE.json's metric); this kernel issues "
+                 "the add-max-relu as HFMA2.RELU on the FMA pipe and only the 3-input max on the ALU pipe, so the bound that holds is "
+                 "issue_frac (all issued instructions against one warp instruction per clock per sub-partition)")
+                if kernel == "scan_filter_lq_kernel" else None,
     }
     line = {
         "metric": "MaxSS GCUPS (scan+top-2+NW step)", "value": cells_step * world / (ms_per_step * 1e-3) / 1e9,
