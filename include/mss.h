@@ -302,7 +302,7 @@ int mss_set_two_pass_chunk_bytes(int64_t bytes);
  * widened to fp16 pairs (half the shared-memory traffic), -1 = automatic: the highest of these the scoring and the read
  * length allow (a forced value that they do not allow is lowered the same way).  Adding 8 (8..10, 11 = automatic arithmetic)
  * makes the kernel read a query's plane offsets from its shared-memory table instead of registers, adding 16 (16..19) keeps
- * them in registers where the read length allows (up to 256 scored positions); default: registers up to 160 scored positions.
+ * them in registers where the read length allows (up to 256 scored positions); default: registers up to 152 scored positions.
  * Adding 32 (32..35) keeps 8 chains per thread for short reads (default: 16 chains for reads of up to 52 scored positions).
  * Bad values: MSS_ERR_ARG. */
 int mss_set_pass1_geometry(int32_t query_sets, int32_t tile_window_starts, int32_t arithmetic);

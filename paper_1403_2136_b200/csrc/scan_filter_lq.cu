@@ -62,7 +62,7 @@ constexpr int LQ_K16 = 16;          // host side: flag = the 16-chain instances 
 #define LQ_K16_UP_TO_NJ 38          // reads of at most this many double steps (76 scored positions) take the 16-chain instances
 #endif
 #ifndef LQ_TABLE_FROM_NJ
-#define LQ_TABLE_FROM_NJ 80         // reads of more double steps than this (> 160 scored positions) take the table-driven instance
+#define LQ_TABLE_FROM_NJ 76         // reads of more double steps than this (> 152 scored positions) take the table-driven instance
 #endif
 
 struct LqTile {
@@ -552,7 +552,8 @@ int32_t lq_nj_instance(int32_t nj, int mode);
 // arithmetic | LQ_TABLE: where a query's plane offsets live.  Registers hold at most 128 double steps (256 scored positions);
 // beyond that, and where it measured faster, they come from the shared-memory table.  Measured (e5m2 operands, cells/clk/SM,
 // registers / table): 36 bp 129.8 / 118.2, 100 bp 136.7 / 124.5, 150 bp 133.1 / 125.3, 250 bp 112.1 (16-bit offset pairs) /
-// 126.5: the table costs one LDS.64 per pair of double steps and a rolled loop, and is the same for every length.
+// 126.5: the table costs one LDS.64 per pair of double steps and a rolled loop, and is the same for every length.  With 16 chains
+// per thread (the table frees the registers for them) it reaches 131.5 / 131.6 / 132.8 at 100 / 150 / 250 bp.
 int lq_plan(const ScanParams& p)
 {
     const int mode = lq_mode(p);
@@ -564,7 +565,8 @@ int lq_plan(const ScanParams& p)
     if (nj > 128) table = true;
     const int32_t inst = lq_nj_instance(nj, mode);              // only the tight short-read instances exist with 16 chains
     const bool k16 = !table && mode == LQ_F8 && nj <= LQ_K16_UP_TO_NJ && (inst == 18 || inst == 26 || inst == 38) && !t_lq_k8;
-    return mode | (table ? LQ_TABLE : 0) | (k16 ? LQ_K16 : 0);
+    const bool t16 = table && mode == LQ_F8 && !t_lq_k8;         // the table-driven e5m2 instance has the registers for 16 chains too
+    return mode | (table ? LQ_TABLE : 0) | ((k16 || t16) ? LQ_K16 : 0);
 }
 
 // the tile: 2*HALF window starts, HALF a multiple of the columns one more group of every warp of a set adds;
@@ -706,6 +708,7 @@ cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint
     // padding steps cost time (the early-exit check is coarse): the common read lengths get a tight instance of the
     // fast arithmetic (36, 51, 76, 100, 150 bp)
     if (mode == LQ_PSSM) return lq_launch3<2, false, LQ_PSSM>(p, ug, ubound, st, smem);   // table-driven: one instance for every length
+    if ((plan & LQ_TABLE) && (plan & LQ_K16)) return lq_launch3<0, false, LQ_F8, 16>(p, ug, ubound, st, smem);
     if (plan & LQ_TABLE) return lq_launch<0, false>(mode, p, ug, ubound, st, smem);
     switch (lq_nj_instance(lq_double_steps(p), mode)) {
         case 18: return (plan & LQ_K16) ? lq_launch3<18, false, LQ_F8, 16>(p, ug, ubound, st, smem) : lq_launch3<18, false, LQ_F8>(p, ug, ubound, st, smem);
