@@ -470,7 +470,7 @@ def plumbing_only(args, cfg, rank: int, world: int) -> None:
     own_ms = 0.0
     for _ in range(args.steps):
         t0 = time.perf_counter()
-        time.sleep(0.005 * (rank + 1))
+        time.sleep(0.05 * (rank + 1))
         own_ms += 1e3 * (time.perf_counter() - t0)
     if world > 1:
         dist.barrier()

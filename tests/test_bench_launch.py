@@ -27,8 +27,8 @@ def test_gpus_2_spawns_two_ranks_and_takes_the_max():
     assert d["n_gpus"] == 2 and d["steps"] == 3 and d["scaling"] == "weak"
     assert d["reads_per_gpu"] == 48                         # weak scaling: every rank maps its own batch of that size
     assert len(d["read_digests"]) == 2 and d["read_digests"][0] != d["read_digests"][1]   # per-rank seeds differ
-    # rank 1 sleeps twice as long as rank 0: the reported time is the slower rank's
-    assert d["ms_per_step"] * 3 > d["own_ms_rank0"] * 1.5
+    # rank 0 "works" 50 ms per step, rank 1 100 ms: the reported time is the slower rank's (sleep never returns early)
+    assert d["ms_per_step"] >= 99.0 and d["ms_per_step"] * 3 >= d["own_ms_rank0"]
 
 
 def test_gpus_1_stays_in_process():
