@@ -14,8 +14,11 @@ def _run(*extra, env_extra=None):
     for k in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT"):
         env.pop(k, None)
     env.update(env_extra or {})
-    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--plumbing-only", "--steps", "3", "--warmup", "1", *extra],
-                       capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--plumbing-only", "--steps", "3", "--warmup", "1", *extra]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    if r.returncode != 0 and ("address already in use" in r.stderr.lower() or "timed out" in r.stderr.lower()):
+        # the rendezvous port is picked free and then bound by the launcher: another process can take it in between; once more
+        r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
     assert len(lines) == 1, r.stdout                       # rank 0 alone prints
