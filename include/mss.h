@@ -18,7 +18,8 @@
  *
  * Conventions
  *   - Every pointer named d_* is DEVICE memory owned by the caller; h_* is HOST memory owned by the caller.
- *     The library allocates no device memory: scratch comes from the caller through the *_workspace_bytes queries.
+ *     The library allocates no device memory: scratch comes from the caller through the *_workspace_bytes queries
+ *     (mss_map_reads_static instead uses a static device array of MSS_STATIC_SCRATCH_BYTES that is part of the library image).
  *     mss_genome_load allocates one small host struct (the handle), released by mss_genome_free; the packed genome
  *     and the genome workspace must outlive the handle.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls enqueue work on it and
@@ -294,7 +295,7 @@ int mss_set_pass_timing(int on);
  * queries follow it.  Results do not depend on it; tests set it small to exercise the chunk loop. */
 int mss_set_two_pass_chunk_bytes(int64_t bytes);
 /* Geometry of the lane-per-query pass-1 kernel (this thread only; results do not depend on it).  query_sets: 32-query
- * sets per block, 1, 2 or 4 (reads per block = 16, 32 or 64 with both strands, twice that with one; 0 = by batch size) --
+ * sets per block, 1, 2 or 4 (reads per block = 16, 32 or 64 with both strands, twice that with one; 0 = automatic) --
  * BASELINE.json config 5's "reads-per-block swept".  tile_window_starts: window starts per tile (even; 0 = automatic:
  * the tile with the least padding of the fragment length that leaves room for two blocks per SM); a value no tile can
  * take makes pass 1 fall back to the tile kernel.  arithmetic: how the chains are computed -- 0 = packed int16 DPX
@@ -303,7 +304,8 @@ int mss_set_two_pass_chunk_bytes(int64_t bytes);
  * length allow (a forced value that they do not allow is lowered the same way).  Adding 8 (8..10, 11 = automatic arithmetic)
  * makes the kernel read a query's plane offsets from its shared-memory table instead of registers, adding 16 (16..19) keeps
  * them in registers where the read length allows (up to 256 scored positions); default: registers up to 152 scored positions.
- * Adding 32 (32..35) keeps 8 chains per thread for short reads (default: 16 chains for reads of up to 52 scored positions).
+ * Adding 32 (32..35) keeps 8 chains per thread where the default is 16 (reads of up to 52 and of 65-76 scored positions, and the
+ * table-driven instance).  query_sets 0 = the most sets with which read groups x fragments still fill the GPU.
  * Bad values: MSS_ERR_ARG. */
 int mss_set_pass1_geometry(int32_t query_sets, int32_t tile_window_starts, int32_t arithmetic);
 int mss_get_pass_times(float *h_pass1_ms, float *h_pass2_ms);
