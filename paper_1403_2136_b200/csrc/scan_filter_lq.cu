@@ -557,7 +557,7 @@ int32_t lq_nj_instance(int32_t nj, int mode);
 int lq_plan(const ScanParams& p)
 {
     const int mode = lq_mode(p);
-    if (mode == LQ_PSSM) return mode;
+    if (mode == LQ_PSSM) return mode | (t_lq_k8 ? 0 : LQ_K16);   // table-driven by construction: registers for 16 chains
     const int32_t nj = lq_double_steps(p);
     bool table = nj > LQ_TABLE_FROM_NJ;
     if (t_lq_table == 1) table = true;
@@ -707,7 +707,8 @@ cudaError_t launch_scan_filter_lq(const mss_genome* g, const ScanParams& p, uint
     if (rpb_out) *rpb_out = ug.reads_per_group;
     // padding steps cost time (the early-exit check is coarse): the common read lengths get a tight instance of the
     // fast arithmetic (36, 51, 76, 100, 150 bp)
-    if (mode == LQ_PSSM) return lq_launch3<2, false, LQ_PSSM>(p, ug, ubound, st, smem);   // table-driven: one instance for every length
+    if (mode == LQ_PSSM)                                                                  // table-driven: one instance for every length
+        return (plan & LQ_K16) ? lq_launch3<2, false, LQ_PSSM, 16>(p, ug, ubound, st, smem) : lq_launch3<2, false, LQ_PSSM>(p, ug, ubound, st, smem);
     if ((plan & LQ_TABLE) && (plan & LQ_K16)) return lq_launch3<0, false, LQ_F8, 16>(p, ug, ubound, st, smem);
     if (plan & LQ_TABLE) return lq_launch<0, false>(mode, p, ug, ubound, st, smem);
     switch (lq_nj_instance(lq_double_steps(p), mode)) {
